@@ -1,0 +1,173 @@
+// common.cuh -- context, launch-parameter structs and small device helpers shared by the kernels of
+// liboci_b200.so. Nothing here is shared with oracle/ (see DESIGN.md "Independence").
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/oci.h"
+
+#define OCI_CUDA_TRY(ctx, expr)                                   \
+    do {                                                          \
+        cudaError_t _e = (expr);                                  \
+        if (_e != cudaSuccess) {                                  \
+            (ctx)->last_cuda = (int)_e;                           \
+            return OCI_E_CUDA;                                    \
+        }                                                         \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------------------
+// Context. All device pointers are carved out of the caller's workspace (the library never cudaMallocs).
+// ------------------------------------------------------------------------------------------------------------
+struct oci_ctx {
+    int J, N, G, n;
+    double dt;
+    int bc_left, bc_right;
+    cudaStream_t stream;
+    int device, num_sms, max_smem_optin;
+    int last_cuda;
+
+    // problem (device copies)
+    double *dx, *sigma_t, *transfer, *v, *mu, *w;
+    // per-step inputs / state
+    double *q;          // [J][G][4]
+    double *inc_left;   // [G][N][2]
+    double *inc_right;  // [G][N][2]
+    double *psi_prev;   // [J][G][N][2]   psi_{k-1/2}
+    double *psi[2];     // [J][n]         Jacobi double buffer; psi[cur] is the current iterate
+    int cur;
+    double *phi;        // [J][G][4]      scalar flux of psi[cur]
+    double *c;          // [J][n]         constant part of b_j (a3)
+    // OCI factors
+    double *Minv;       // [J][n(col)][n(row)]  A_j^{-1}, column-major per cell
+    double *scratch;    // factor kernel scratch (n > smem capacity) / debug matrix
+    size_t scratch_bytes;
+    int *info;          // [1] singular-cell flag (min 1-based cell index, INT_MAX = none)
+    // SI data
+    double *si_Linv;    // [J][G][N][16]  inverse of L_{c,j,g,m} (Eq. 42)
+    double *si_T;       // [J][G*N][4][2] C = |mu| Linv[:, incident rows]; its outgoing rows are the sweep's 2x2 map
+    double *si_base;    // [J][G*N][4]    Linv * d (no incident term)
+    double *si_in;      // [J][G*N][2]    incident edge flux of cell j found by the sweep
+    // residual history (device) + pinned host mirror
+    unsigned long long *resid_inf; // [OCI_RESID_CAP] bit pattern of a non-negative double
+    double *resid_l2;              // [OCI_RESID_CAP] sum of squares
+    double *h_resid;               // pinned host, 2 * OCI_RESID_CAP
+    int hist_len;                  // iterations recorded since the history was last reset
+    int hist_has_l2;
+
+    bool factored, c_valid, si_valid, phi_valid;
+    // options
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph;
+    // timing
+    cudaEvent_t ev0, ev1;
+    double last_ms[3];
+    long long last_launches[3];
+};
+
+// ------------------------------------------------------------------------------------------------------------
+// Kernel parameter blocks
+// ------------------------------------------------------------------------------------------------------------
+struct ProblemView {
+    int J, N, G, n;
+    double dt;
+    int bc_left, bc_right;
+    const double *dx, *sigma_t, *transfer, *v, *mu, *w;
+};
+
+struct IterParams {
+    int J, N, G, n;
+    int bc_left, bc_right;
+    const double *Minv;
+    const double *c;
+    const double *psi_old;
+    double *psi_new;
+    double *phi;
+    const double *mu, *w;
+    const double *inc_left, *inc_right;
+    unsigned long long *resid_inf; // slot of this iteration
+    double *resid_l2;              // slot of this iteration (nullptr: not recorded)
+    // work decomposition of the pipelined kernel
+    int cpb;      // cells per work item (> 1 only when a whole item fits one chunk)
+    int S;        // column sub-groups per cell team
+    int cw;       // columns per chunk (cpb == 1)
+    int nch;      // chunks per item
+    int n_items;
+    int stages;   // matrix ring depth
+    int chunk_doubles;
+};
+
+static inline ProblemView make_view(const oci_ctx *c)
+{
+    ProblemView p;
+    p.J = c->J; p.N = c->N; p.G = c->G; p.n = c->n; p.dt = c->dt;
+    p.bc_left = c->bc_left; p.bc_right = c->bc_right;
+    p.dx = c->dx; p.sigma_t = c->sigma_t; p.transfer = c->transfer; p.v = c->v; p.mu = c->mu; p.w = c->w;
+    return p;
+}
+
+// launchers implemented in the kernel translation units (each returns the number of kernels launched, < 0 on error)
+int launch_factor(oci_ctx *ctx);
+int launch_assemble_one(oci_ctx *ctx, int cell, double *A_dev_rowmajor);
+int launch_const_rhs(oci_ctx *ctx);
+int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2);
+int launch_advance(oci_ctx *ctx);
+int launch_seed_iterate(oci_ctx *ctx);
+int launch_scalar_flux(oci_ctx *ctx, const double *psi, double *phi);
+int launch_si_setup(oci_ctx *ctx);
+int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2);
+
+#ifdef __CUDACC__
+// ------------------------------------------------------------------------------------------------------------
+// Device helpers
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// non-negative doubles order like their bit patterns; NaN is mapped to +inf so it is never lost
+__device__ __forceinline__ unsigned long long resid_bits(double d)
+{
+    if (!(d == d)) d = __longlong_as_double(0x7ff0000000000000LL);
+    return (unsigned long long)__double_as_longlong(d);
+}
+
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        double u = __shfl_xor_sync(0xffffffffu, v, o);
+        v = (u > v || !(u == u)) ? u : v;
+    }
+    return v;
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Eq. 8b, PAPER.md:132 -- entry (p, pp) of the 4x4 within-cell block L_{c,j,g,m}. Every operation is an
+// explicitly rounded intrinsic so that the assembled matrix is bit-identical to a plain (uncontracted)
+// evaluation of the same formula.
+__device__ __forceinline__ double lc_entry(int p, int pp, double dx, double sig, double v, double dt, double mu)
+{
+    const double a = __dmul_rn(__dadd_rn(fabs(mu), __dmul_rn(dx, sig)), 0.5); // (|mu| + dx Sigma)/2
+    const double gam = __ddiv_rn(dx, __dmul_rn(v, dt));                       // dx / (v dt)
+    const double h = __dmul_rn(mu, 0.5);
+    const int e = p * 4 + pp;
+    switch (e) {
+    case 0:  return a;
+    case 1:  return h;
+    case 2:  return __dmul_rn(gam, 0.5);
+    case 4:  return -h;
+    case 5:  return a;
+    case 7:  return __dmul_rn(gam, 0.5);
+    case 8:  return -gam;
+    case 10: return __dadd_rn(gam, a);
+    case 11: return h;
+    case 13: return -gam;
+    case 14: return -h;
+    case 15: return __dadd_rn(gam, a);
+    default: return 0.0;
+    }
+}
+#endif

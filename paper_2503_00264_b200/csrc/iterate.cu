@@ -1,0 +1,515 @@
+// iterate.cu -- a3..a8 of SURVEY.md section 8(a): constant RHS, the fused per-iteration OCI kernel
+// (gather incident edge fluxes + RHS + cell solve + scalar flux + residual), advance.
+//
+// One OCI iteration (Eq. 7; Alg. 2), for every cell j independently:
+//   b_j = c_j + incident(Psi^(l))    Eq. 9c-d: rows (k,L),(k+1/2,L) of an ordinate with mu>0 get
+//                                    +mu psi^(l)_{j-1,R}; rows (k,R),(k+1/2,R) of mu<0 get +|mu| psi^(l)_{j+1,L}
+//   Psi_j^(l+1) = A_j^{-1} b_j       the `_getrs` of Alg. 2, here a streamed matrix-vector product with the
+//                                    inverse oci_factor stored (same n^2 doubles, same 2 n^2 flops, no chain)
+//   phi_j = sum_m w_m psi_m          Eq. 44
+//   r = max |phi^(l+1) - phi^(l)|    (and sum (Psi^(l+1)-Psi^(l))^2 for Eq. 12)
+// The kernel is HBM-bound: 8 n^2 bytes of A_j^{-1} per cell-solve against 2 n^2 flops. It therefore runs as
+// a persistent, warp-specialised streaming kernel: one producer thread per CTA issues 1-D bulk async copies
+// (cp.async.bulk, completion on mbarriers) into a multi-stage shared-memory ring; eight consumer warps
+// multiply the chunks as they land.
+#include "common.cuh"
+
+namespace {
+
+constexpr int CONSUMER_WARPS = 8;
+constexpr int CONSUMERS = CONSUMER_WARPS * 32;       // 256
+constexpr int ITER_THREADS = CONSUMERS + 32;         // + 1 producer warp
+constexpr int VEC_SLOTS = 2;
+constexpr int MAX_STAGES = 8;
+
+// ---- mbarrier / bulk-copy PTX wrappers ---------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// Bounded wait: a protocol bug traps (-> CUDA error) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    unsigned long long t0 = 0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if ((++spins & 0x3ff) == 0) {
+            unsigned long long t1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+            if (t1 - t0 > 4000000000ULL) __trap(); // 4 s
+        }
+    }
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void consumer_bar()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(CONSUMERS) : "memory");
+}
+
+// ---- incident edge flux of entry (cell j, row i) taken from Psi^(l) ------------------------------------------
+// `nb` holds Psi^(l) of cells j0-1 .. j0+nc (cell j at nb + (j - j0 + 1) * n); returns coefficient * value.
+__device__ __forceinline__ double incident_term(const IterParams &P, const double *nb, int j0, int j, int i,
+                                                const double *mu_s)
+{
+    const int n = P.n, N = P.N;
+    const int p = i & 3, bm = i >> 2, m = bm % N, g = bm / N;
+    const double mu = mu_s[m];
+    const double *self = nb + (size_t)(j - j0 + 1) * n;
+    if (mu > 0.0 && !(p & 1)) { // rows (k,L), (k+1/2,L): upstream = (j-1, R), Eq. 5a / 9c
+        double val;
+        if (j > 0) val = (self - n)[i + 1];
+        else if (P.bc_left == OCI_BC_REFLECTIVE) val = self[(g * N + (N - 1 - m)) * 4 + p];
+        else if (P.bc_left == OCI_BC_PRESCRIBED) val = P.inc_left[(g * N + m) * 2 + (p >> 1)];
+        else val = 0.0;
+        return mu * val;
+    }
+    if (mu < 0.0 && (p & 1)) { // rows (k,R), (k+1/2,R): upstream = (j+1, L), Eq. 5b / 9d
+        double val;
+        if (j < P.J - 1) val = (self + n)[i - 1];
+        else if (P.bc_right == OCI_BC_REFLECTIVE) val = self[(g * N + (N - 1 - m)) * 4 + p];
+        else if (P.bc_right == OCI_BC_PRESCRIBED) val = P.inc_right[(g * N + m) * 2 + (p >> 1)];
+        else val = 0.0;
+        return -mu * val;
+    }
+    return 0.0;
+}
+
+// ============================================================================================================
+// Pipelined streaming kernel
+// ============================================================================================================
+// Work item = `cpb` consecutive cells (cpb > 1 only for small n, where several whole inverses fit one chunk)
+// = `nch` chunks of the inverse (column panels of `cw` columns when one cell spans several chunks).
+// Consumer thread t of a cell team (team size n*S) owns row r = t % n and the columns c = sub (mod S),
+// sub = t / n: with the column-major inverse every step of a team reads S*n consecutive doubles, so shared
+// memory reads are conflict-free and the global layout needs no swizzle.
+template <bool WANT_L2>
+__global__ void __launch_bounds__(ITER_THREADS, 1) oci_iterate_stream_kernel(const IterParams P)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int n = P.n, N = P.N, G = P.G, J = P.J;
+    const int cpb = P.cpb, S = P.S, nch = P.nch, stages = P.stages;
+    const int vec_c = cpb * n, vec_nb = (cpb + 2) * n;
+
+    uint64_t *mat_full = reinterpret_cast<uint64_t *>(smem_raw);
+    uint64_t *mat_empty = mat_full + MAX_STAGES;
+    uint64_t *vec_full = mat_empty + MAX_STAGES;
+    uint64_t *vec_empty = vec_full + VEC_SLOTS;
+    double *mu_s = reinterpret_cast<double *>(vec_empty + VEC_SLOTS); // [N]
+    double *w_s = mu_s + N;                                          // [N]
+    double *part = w_s + N;                                          // [CONSUMERS]
+    double *xbuf = part + CONSUMERS;                                 // [CONSUMERS]
+    size_t off = (size_t)((unsigned char *)(xbuf + CONSUMERS) - smem_raw);
+    off = (off + 127) & ~(size_t)127;
+    double *vec = reinterpret_cast<double *>(smem_raw + off);        // VEC_SLOTS x (vec_c + vec_nb)
+    off += (size_t)VEC_SLOTS * (vec_c + vec_nb) * sizeof(double);
+    off = (off + 127) & ~(size_t)127;
+    double *mat = reinterpret_cast<double *>(smem_raw + off);        // stages x chunk_doubles
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    if (tid == 0) {
+        for (int s = 0; s < stages; ++s) { mbar_init(&mat_full[s], 1); mbar_init(&mat_empty[s], CONSUMER_WARPS); }
+        for (int s = 0; s < VEC_SLOTS; ++s) { mbar_init(&vec_full[s], 1); mbar_init(&vec_empty[s], CONSUMER_WARPS); }
+        fence_mbar_init();
+    }
+    for (int i = tid; i < N; i += ITER_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    __syncthreads();
+
+    // balanced contiguous split of the items over the CTAs
+    const int item0 = (int)(((long long)P.n_items * blockIdx.x) / gridDim.x);
+    const int item1 = (int)(((long long)P.n_items * (blockIdx.x + 1)) / gridDim.x);
+
+    if (warp == CONSUMER_WARPS) {
+        // ===================== producer: one thread issues every bulk copy ===============================
+        if (lane == 0) {
+            int ms = 0, vs = 0;
+            uint32_t mph = 0, vph = 0;
+            for (int item = item0; item < item1; ++item) {
+                const int j0 = item * cpb;
+                const int nc = min(cpb, J - j0);
+                // vectors: c_j of the item's cells, Psi^(l) of the cells and their two neighbours
+                mbar_wait(&vec_empty[vs], vph ^ 1);
+                {
+                    double *cs = vec + (size_t)vs * (vec_c + vec_nb);
+                    double *nb = cs + vec_c;
+                    const int lo = max(j0 - 1, 0), hi = min(j0 + nc, J - 1);
+                    const uint32_t bytes_c = (uint32_t)(nc * n * sizeof(double));
+                    const uint32_t bytes_nb = (uint32_t)((hi - lo + 1) * n * sizeof(double));
+                    mbar_arrive_expect_tx(&vec_full[vs], bytes_c + bytes_nb);
+                    bulk_g2s(cs, P.c + (size_t)j0 * n, bytes_c, &vec_full[vs]);
+                    bulk_g2s(nb + (size_t)(lo - (j0 - 1)) * n, P.psi_old + (size_t)lo * n, bytes_nb, &vec_full[vs]);
+                }
+                if (++vs == VEC_SLOTS) { vs = 0; vph ^= 1; }
+                // matrix chunks
+                const double *src0 = P.Minv + (size_t)j0 * n * n;
+                for (int ch = 0; ch < nch; ++ch) {
+                    mbar_wait(&mat_empty[ms], mph ^ 1);
+                    uint32_t bytes;
+                    const double *src;
+                    if (nch == 1) { src = src0; bytes = (uint32_t)((size_t)nc * n * n * sizeof(double)); }
+                    else {
+                        const int c0 = ch * P.cw, ncol = min(P.cw, n - c0);
+                        src = src0 + (size_t)c0 * n;
+                        bytes = (uint32_t)((size_t)ncol * n * sizeof(double));
+                    }
+                    mbar_arrive_expect_tx(&mat_full[ms], bytes);
+                    bulk_g2s(mat + (size_t)ms * P.chunk_doubles, src, bytes, &mat_full[ms]);
+                    if (++ms == stages) { ms = 0; mph ^= 1; }
+                }
+            }
+        }
+        return;
+    }
+
+    // ========================= consumers ====================================================================
+    const int TS = n * S;                 // threads of one cell team
+    const int team = tid / TS;            // cell within the item
+    const int tt = tid - team * TS;
+    const int sub = tt / n, r = tt - sub * n;
+    const bool in_team = team < cpb;      // false: idle in the product phase (n*S*cpb < 256)
+
+    int ms = 0, vs = 0;
+    uint32_t mph = 0, vph = 0;
+    double rmax = 0.0, l2 = 0.0;
+
+    for (int item = item0; item < item1; ++item) {
+        const int j0 = item * cpb;
+        const int nc = min(cpb, J - j0);
+        double *cs = vec + (size_t)vs * (vec_c + vec_nb);
+        const double *nb = cs + vec_c;
+
+        // ---- a4: b = c + incident(Psi^(l)), in place over c
+        mbar_wait(&vec_full[vs], vph);
+        for (int e = tid; e < nc * n; e += CONSUMERS) {
+            const int a = e / n, i = e - a * n;
+            cs[e] += incident_term(P, nb, j0, j0 + a, i, mu_s);
+        }
+        consumer_bar();
+
+        // ---- a5: x = A^{-1} b, chunk by chunk
+        double acc0 = 0.0, acc1 = 0.0;
+        for (int ch = 0; ch < nch; ++ch) {
+            mbar_wait(&mat_full[ms], mph);
+            if (in_team && team < nc) {
+                int c0 = 0, ncol = n;
+                if (nch > 1) { c0 = ch * P.cw; ncol = min(P.cw, n - c0); }
+                const double *Mp = mat + (size_t)ms * P.chunk_doubles + (size_t)team * n * n + r;
+                const double *bp = cs + team * n + c0;
+                int cc = sub;
+#pragma unroll 4
+                for (; cc + S < ncol; cc += 2 * S) {
+                    acc0 = fma(Mp[(size_t)cc * n], bp[cc], acc0);
+                    acc1 = fma(Mp[(size_t)(cc + S) * n], bp[cc + S], acc1);
+                }
+                if (cc < ncol) acc0 = fma(Mp[(size_t)cc * n], bp[cc], acc0);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&mat_empty[ms]);
+            if (++ms == stages) { ms = 0; mph ^= 1; }
+        }
+        part[tid] = acc0 + acc1;
+        consumer_bar();
+
+        // ---- combine the column sub-groups; write Psi^(l+1)
+        for (int e = tid; e < nc * n; e += CONSUMERS) {
+            const int a = e / n, i = e - a * n;
+            double x = 0.0;
+            for (int s = 0; s < S; ++s) x += part[a * TS + s * n + i];
+            xbuf[e] = x;
+            P.psi_new[(size_t)j0 * n + e] = x;
+            if (WANT_L2) { const double d = x - nb[(a + 1) * n + i]; l2 = fma(d, d, l2); }
+        }
+        consumer_bar();
+
+        // ---- a6 + a7: phi = sum_m w_m psi_m for the new and the previous iterate, residual
+        for (int e = tid; e < nc * G * 4; e += CONSUMERS) {
+            const int p = e & 3, ag = e >> 2, g = ag % G, a = ag / G;
+            const double *xn = xbuf + a * n + g * N * 4 + p;
+            const double *xo = nb + (a + 1) * n + g * N * 4 + p;
+            double sn = 0.0, so = 0.0;
+            for (int m = 0; m < N; ++m) { sn = fma(w_s[m], xn[m * 4], sn); so = fma(w_s[m], xo[m * 4], so); }
+            P.phi[(size_t)j0 * G * 4 + e] = sn;
+            const double d = fabs(sn - so);
+            rmax = (d > rmax || !(d == d)) ? d : rmax;
+        }
+        // the slot was written through the generic proxy (b in place of c) and is refilled by bulk copies
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&vec_empty[vs]);
+        if (++vs == VEC_SLOTS) { vs = 0; vph ^= 1; }
+    }
+
+    rmax = warp_max(rmax);
+    if (lane == 0 && item1 > item0) atomicMax(P.resid_inf, resid_bits(rmax));
+    if (WANT_L2) {
+        l2 = warp_sum(l2);
+        if (lane == 0 && item1 > item0) atomicAdd(P.resid_l2, l2);
+    }
+}
+
+// ============================================================================================================
+// Plain kernel: one CTA per cell, loads straight from global memory. Used for cross-checking the pipelined
+// kernel and selectable with oci_set_option("iterate_kernel", 0).
+// ============================================================================================================
+template <bool WANT_L2>
+__global__ void __launch_bounds__(256) oci_iterate_plain_kernel(const IterParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n = P.n, N = P.N, G = P.G, J = P.J;
+    double *b = reinterpret_cast<double *>(smem_raw); // [n]
+    double *x = b + n;                                // [n]
+    double *nb = x + n;                               // [3n] Psi^(l) of cells j-1, j, j+1
+    double *mu_s = nb + 3 * n;                        // [N]
+    double *w_s = mu_s + N;
+    const int tid = threadIdx.x, lane = tid & 31;
+    for (int i = tid; i < N; i += blockDim.x) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    double rmax = 0.0, l2 = 0.0;
+    for (int j = blockIdx.x; j < J; j += gridDim.x) {
+        __syncthreads();
+        for (int e = tid; e < 3 * n; e += blockDim.x) {
+            const int jj = j - 1 + e / n;
+            nb[e] = (jj >= 0 && jj < J) ? P.psi_old[(size_t)jj * n + (e % n)] : 0.0;
+        }
+        __syncthreads();
+        for (int i = tid; i < n; i += blockDim.x) b[i] = P.c[(size_t)j * n + i] + incident_term(P, nb, j, j, i, mu_s);
+        __syncthreads();
+        const double *M = P.Minv + (size_t)j * n * n;
+        for (int i = tid; i < n; i += blockDim.x) {
+            double acc = 0.0;
+            for (int c = 0; c < n; ++c) acc = fma(M[(size_t)c * n + i], b[c], acc);
+            x[i] = acc;
+            P.psi_new[(size_t)j * n + i] = acc;
+            if (WANT_L2) { const double d = acc - nb[n + i]; l2 = fma(d, d, l2); }
+        }
+        __syncthreads();
+        for (int e = tid; e < G * 4; e += blockDim.x) {
+            const int p = e & 3, g = e >> 2;
+            double sn = 0.0, so = 0.0;
+            for (int m = 0; m < N; ++m) {
+                sn = fma(w_s[m], x[(g * N + m) * 4 + p], sn);
+                so = fma(w_s[m], nb[n + (g * N + m) * 4 + p], so);
+            }
+            P.phi[(size_t)j * G * 4 + e] = sn;
+            const double d = fabs(sn - so);
+            rmax = (d > rmax || !(d == d)) ? d : rmax;
+        }
+    }
+    rmax = warp_max(rmax);
+    if (lane == 0) atomicMax(P.resid_inf, resid_bits(rmax));
+    if (WANT_L2) {
+        l2 = warp_sum(l2);
+        if (lane == 0) atomicAdd(P.resid_l2, l2);
+    }
+}
+
+// ---- a3: constant part of b_j (Eq. 9c-d without the incident terms; 4th row of 9c restored,
+// DESIGN.md A1): rows (k,L),(k,R): dx/4 Q_k + dx/(2 v dt) psi_{k-1/2}; rows (k+1/2,L),(k+1/2,R): dx/4 Q_{k+1/2}
+__global__ void const_rhs_kernel(ProblemView P, const double *__restrict__ q, const double *__restrict__ psi_prev,
+                                 double *__restrict__ c)
+{
+    const size_t total = (size_t)P.J * P.n;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+        const int p = (int)(e & 3);
+        const size_t jgm = e >> 2;
+        const size_t jg = jgm / P.N;
+        const int g = (int)(jg % P.G);
+        const size_t j = jg / P.G;
+        const double dx = P.dx[j];
+        double val = dx * 0.25 * q[jg * 4 + p];
+        if (p < 2) val += dx / (2.0 * P.v[g] * P.dt) * psi_prev[jgm * 2 + p];
+        c[e] = val;
+    }
+}
+
+// ---- a8: psi_{k-1/2} <- psi_{k+1/2} of the converged iterate
+__global__ void advance_kernel(size_t n_pairs, const double *__restrict__ psi, double *__restrict__ psi_prev)
+{
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_pairs * 2; e += (size_t)gridDim.x * blockDim.x)
+        psi_prev[e] = psi[(e >> 1) * 4 + 2 + (e & 1)];
+}
+
+// iterate <- both time levels = psi_{k-1/2} (A11)
+__global__ void seed_iterate_kernel(size_t n_pairs, const double *__restrict__ psi_prev, double *__restrict__ psi)
+{
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_pairs * 4; e += (size_t)gridDim.x * blockDim.x)
+        psi[e] = psi_prev[(e >> 2) * 2 + (e & 1)];
+}
+
+// Eq. 44: phi[j][g][p] = sum_m w_m psi[j][g][m][p]
+__global__ void scalar_flux_kernel(int J, int N, int G, const double *__restrict__ w, const double *__restrict__ psi,
+                                   double *__restrict__ phi)
+{
+    const size_t total = (size_t)J * G * 4;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+        const int p = (int)(e & 3);
+        const size_t jg = e >> 2;
+        double s = 0.0;
+        for (int m = 0; m < N; ++m) s = fma(w[m], psi[(jg * N + m) * 4 + p], s);
+        phi[e] = s;
+    }
+}
+
+inline int grid_for(size_t total, int threads, int num_sms)
+{
+    size_t g = (total + threads - 1) / threads;
+    size_t cap = (size_t)num_sms * 16;
+    if (g > cap) g = cap;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+} // namespace
+
+// ------------------------------------------------------------------------------------------------------------
+// Work decomposition of the pipelined kernel for a given n (host side)
+// ------------------------------------------------------------------------------------------------------------
+struct StreamPlan {
+    int cpb, S, cw, nch, chunk_doubles, stages, grid;
+    size_t smem;
+};
+
+static StreamPlan make_plan(const oci_ctx *ctx)
+{
+    StreamPlan pl;
+    const int n = ctx->n;
+    const int CH = 4096; // doubles per chunk (32 KB)
+    int cpb = CH / (n * n);
+    if (cpb < 1) cpb = 1;
+    if (cpb > CONSUMERS / n) cpb = CONSUMERS / n;
+    if (cpb < 1) cpb = 1;
+    pl.cpb = cpb;
+    pl.S = CONSUMERS / (cpb * n);
+    if (pl.S < 1) pl.S = 1;
+    if (cpb > 1 || n * n <= CH) { pl.cw = n; pl.nch = 1; pl.chunk_doubles = cpb * n * n; }
+    else {
+        pl.cw = CH / n;
+        pl.nch = (n + pl.cw - 1) / pl.cw;
+        pl.chunk_doubles = pl.cw * n;
+    }
+    pl.chunk_doubles = (pl.chunk_doubles + 15) & ~15; // keep stages 128-byte aligned
+    const int n_items = (ctx->J + cpb - 1) / cpb;
+    int ctas_per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : 1;
+    const size_t fixed = (size_t)(2 * MAX_STAGES + 2 * VEC_SLOTS) * 8 + (size_t)(2 * ctx->N + 2 * CONSUMERS) * 8 + 256 +
+                         (size_t)VEC_SLOTS * ((2 * cpb + 2) * n) * 8 + 128;
+    const size_t budget = (size_t)ctx->max_smem_optin / ctas_per_sm - (ctas_per_sm > 1 ? 1024 : 0);
+    int stages = (int)((budget - fixed) / ((size_t)pl.chunk_doubles * 8));
+    if (stages > MAX_STAGES) stages = MAX_STAGES;
+    if (ctx->opt_stages > 0 && ctx->opt_stages < stages) stages = ctx->opt_stages;
+    if (stages < 2) stages = 2;
+    pl.stages = stages;
+    pl.smem = fixed + (size_t)stages * pl.chunk_doubles * 8;
+    int grid = ctx->num_sms * ctas_per_sm;
+    if (grid > n_items) grid = n_items;
+    pl.grid = grid;
+    return pl;
+}
+
+int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2)
+{
+    IterParams P;
+    P.J = ctx->J; P.N = ctx->N; P.G = ctx->G; P.n = ctx->n;
+    P.bc_left = ctx->bc_left; P.bc_right = ctx->bc_right;
+    P.Minv = ctx->Minv; P.c = ctx->c;
+    P.psi_old = ctx->psi[ctx->cur]; P.psi_new = ctx->psi[ctx->cur ^ 1];
+    P.phi = ctx->phi; P.mu = ctx->mu; P.w = ctx->w;
+    P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
+    P.resid_inf = ctx->resid_inf + hist_slot;
+    P.resid_l2 = ctx->resid_l2 + hist_slot;
+    if (ctx->opt_iterate_kernel == 0 || ctx->n > CONSUMERS) {
+        P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
+        const size_t smem = (size_t)(5 * ctx->n + 2 * ctx->N) * sizeof(double);
+        int grid = ctx->num_sms * 8;
+        if (grid > ctx->J) grid = ctx->J;
+        if (want_l2) oci_iterate_plain_kernel<true><<<grid, 256, smem, ctx->stream>>>(P);
+        else oci_iterate_plain_kernel<false><<<grid, 256, smem, ctx->stream>>>(P);
+    } else {
+        const StreamPlan pl = make_plan(ctx);
+        P.cpb = pl.cpb; P.S = pl.S; P.cw = pl.cw; P.nch = pl.nch; P.stages = pl.stages;
+        P.chunk_doubles = pl.chunk_doubles;
+        P.n_items = (ctx->J + pl.cpb - 1) / pl.cpb;
+        static size_t attr_set[2] = {0, 0};
+        if (attr_set[want_l2] < pl.smem) {
+            if (want_l2)
+                OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(oci_iterate_stream_kernel<true>,
+                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+            else
+                OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(oci_iterate_stream_kernel<false>,
+                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+            attr_set[want_l2] = pl.smem;
+        }
+        if (want_l2) oci_iterate_stream_kernel<true><<<pl.grid, ITER_THREADS, pl.smem, ctx->stream>>>(P);
+        else oci_iterate_stream_kernel<false><<<pl.grid, ITER_THREADS, pl.smem, ctx->stream>>>(P);
+    }
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    ctx->cur ^= 1;
+    return 1;
+}
+
+int launch_const_rhs(oci_ctx *ctx)
+{
+    ProblemView P = make_view(ctx);
+    const size_t total = (size_t)ctx->J * ctx->n;
+    const_rhs_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(P, ctx->q, ctx->psi_prev, ctx->c);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}
+
+int launch_advance(oci_ctx *ctx)
+{
+    const size_t pairs = (size_t)ctx->J * ctx->G * ctx->N;
+    advance_kernel<<<grid_for(pairs * 2, 256, ctx->num_sms), 256, 0, ctx->stream>>>(pairs, ctx->psi[ctx->cur],
+                                                                                      ctx->psi_prev);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}
+
+int launch_seed_iterate(oci_ctx *ctx)
+{
+    const size_t pairs = (size_t)ctx->J * ctx->G * ctx->N;
+    seed_iterate_kernel<<<grid_for(pairs * 4, 256, ctx->num_sms), 256, 0, ctx->stream>>>(pairs, ctx->psi_prev,
+                                                                                           ctx->psi[ctx->cur]);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}
+
+int launch_scalar_flux(oci_ctx *ctx, const double *psi, double *phi)
+{
+    const size_t total = (size_t)ctx->J * ctx->G * 4;
+    scalar_flux_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(ctx->J, ctx->N, ctx->G, ctx->w, psi, phi);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}

@@ -1,0 +1,187 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle, element by
+element on the same seeded inputs. Tolerances (BASELINE.json north_star):
+  * assembled A_j: bit-exact (every rounding in the kernel is explicit);
+  * per-iteration angular flux: max|psi_gpu - psi_orc| / max|psi_orc| <= 1e-11 after the same number of iterations;
+  * converged scalar flux: <= 1e-9 relative, GPU and oracle run for the same number of iterations.
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_ITER = 1e-11
+TOL_PHI = 1e-9
+
+
+def _solver(p, **kw):
+    from paper_2503_00264_b200 import OCISolver
+    return OCISolver(p, **kw)
+
+
+def _oracle(p):
+    from oracle import Oracle
+    return Oracle(p)
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
+SMALL_CASES = [
+    # seed, J, N, G, bc_left, bc_right   (n = 4NG: 8, 16, 24, 32, 48, 64, 96, 128, 160, 256; ragged J everywhere)
+    (1, 5, 2, 1, 0, 0),
+    (2, 37, 4, 1, 0, 0),
+    (3, 19, 2, 3, 1, 0),
+    (4, 67, 8, 1, 2, 2),
+    (5, 23, 6, 2, 0, 1),
+    (6, 301, 16, 1, 1, 1),
+    (7, 9, 8, 3, 2, 0),
+    (8, 150, 8, 4, 0, 0),
+    (9, 7, 10, 4, 0, 2),
+    (10, 11, 8, 8, 1, 0),
+    (11, 1, 4, 2, 0, 0),      # a single cell: both neighbours are boundaries
+    (12, 2, 2, 1, 1, 1),
+]
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
+def test_assembly_bit_exact(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p), _oracle(p)
+    for j in sorted({0, J // 2, J - 1}):
+        A_gpu = s.debug_matrix(j)
+        A_orc = o.assemble_cell(j)
+        assert np.array_equal(A_gpu, A_orc), f"cell {j}: max diff {np.max(np.abs(A_gpu - A_orc))}"
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
+def test_factor_gives_inverse(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br, dt=10.0 ** (-(seed % 4)))
+    s, o = _solver(p), _oracle(p)
+    assert s.factor() == 0
+    for j in sorted({0, J // 3, J - 1}):
+        A = o.assemble_cell(j)
+        Ainv = s.debug_inverse(j)
+        n = A.shape[0]
+        assert np.max(np.abs(A @ Ainv - np.eye(n))) < 1e-12 * np.linalg.cond(A)
+
+
+def test_factor_flags_singular_cell():
+    p = W.random_problem(21, 12, 4, 1)
+    p.sigma_t = p.sigma_t.copy()
+    p.sigma_t[7] = np.nan
+    s = _solver(p)
+    assert s.factor() == 8  # 1-based index of the first bad cell
+
+
+@pytest.mark.parametrize("kernel", [1, 0])
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
+def test_oci_per_iteration_parity(seed, J, N, G, bl, br, kernel):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p, options={"iterate_kernel": kernel}), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    assert rel(s.debug_const_rhs().cpu().numpy(), o.c) < 1e-14
+    for l in range(6):
+        s.iterate(1)
+        o.oci_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+    s.iterate(7)
+    o.oci_iterate(7)
+    assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
+def test_si_per_iteration_parity(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p), _oracle(p)
+    for l in range(5):
+        s.si_iterate(1)
+        o.si_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("scheme", ["oci", "si"])
+def test_step_loop_matches_oracle(scheme, rule):
+    """Several time steps: iteration counts (check_every = 1 -> natural count), residual history, converged phi."""
+    p = W.random_problem(31, 40, 4, 2, bc_left=1, bc_right=2, dt=0.05)
+    s, o = _solver(p), _oracle(p)
+    for step in range(3):
+        if scheme == "oci":
+            it_g, conv_g, res_g = s.step(tol=1e-9, max_iters=500, check_every=1, stop_rule=rule)
+            it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule)
+        else:
+            it_g, conv_g, res_g = s.si_step(tol=1e-9, max_iters=500, check_every=1, stop_rule=rule)
+            it_o, hist_o = o.si_step(tol=1e-9, max_iters=500, rule=rule)
+        assert it_g == it_o == conv_g, f"step {step}"
+        hist_g = s.residual_history(kind=rule)
+        assert len(hist_g) == it_o
+        np.testing.assert_allclose(hist_g, hist_o, rtol=1e-6, atol=1e-15)
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+def test_check_every_overshoot_is_bounded_and_same_iterations_agree():
+    """with check_every = k the GPU may run < k extra iterations; the oracle run for exactly that many
+    iterations agrees to 1e-9."""
+    p = W.config2(dt=0.1, J=256)
+    s, o = _solver(p), _oracle(p)
+    it_g, conv_g, _ = s.step(tol=1e-8, max_iters=4000, check_every=8, advance=False)
+    o2 = _oracle(p)
+    it_nat, _ = o2.oci_step(tol=1e-8, max_iters=4000, advance=False)
+    assert conv_g == it_nat
+    assert 0 <= it_g - it_nat < 8
+    o.factor()
+    o.const_rhs()
+    o.oci_iterate(it_g)
+    assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+
+
+def test_config1_full_run_both_schemes():
+    p = W.config1()
+    s, o = _solver(p), _oracle(p)
+    s2, o2 = _solver(p), _oracle(p)
+    for step in range(p.n_steps):
+        it_g, conv_g, _ = s.step(tol=p.tol, check_every=1)
+        it_o, _ = o.oci_step(tol=p.tol)
+        assert it_g == it_o
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+        it_g2, _, _ = s2.si_step(tol=p.tol, check_every=1)
+        it_o2, _ = o2.si_step(tol=p.tol)
+        assert it_g2 == it_o2
+        assert rel(s2.scalar_flux().cpu().numpy(), o2.phi) < TOL_PHI
+
+
+def test_set_iterate_worked_example_head():
+    """Random initial iterate (PAPER.md:479 verification run), no source: the iterate itself is the error."""
+    p = W.worked_example(J=200)
+    s, o = _solver(p), _oracle(p)
+    s.set_iterate(p.meta["psi_guess"])
+    o.set_iterate(p.meta["psi_guess"])
+    s.factor(); o.factor(); o.const_rhs()
+    s.iterate(25)
+    o.oci_iterate(25)
+    assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+def test_set_dt_refactors():
+    p = W.random_problem(41, 30, 4, 2)
+    s = _solver(p)
+    s.factor()
+    s.iterate(3)
+    s.set_dt(p.dt / 10)
+    with pytest.raises(Exception):
+        s.iterate(1)  # factors are stale: OCI_E_STATE
+    s.factor()
+    o = _oracle(p.with_dt(p.dt / 10))
+    o.set_iterate(s.angular_flux().cpu().numpy())
+    o.factor(); o.const_rhs()
+    s.iterate(2)
+    o.oci_iterate(2)
+    assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
