@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- the headline benchmark of this repository (contract: task prompt / DESIGN.md "Measurement").
+
+Metric (BASELINE.json): OCI fp64 cell-solves/s, seconds per converged time step and iterations, OCI vs the GPU SI
+sweep, across a dt sweep, on one B200.
+
+Workload: BASELINE.json configs[4] ("config 5"): single group, S16 (n = 64), 65536 cells, per-cell sigma_t
+log-uniform in [0.01, 100]/cm, c ~ U[0.5, 0.999], dt sweep {1, 1e-1, 1e-2, 1e-3, 1e-4} -- the config the metric's
+"OCI vs GPU SI ... across a dt sweep" is spelled out on, and the largest one (2.1 GB of per-cell inverses, 17x the
+L2, so no L2 flush is needed between iterations). Synthetic, seeded (workloads.config5, seed 1005).
+
+A "step" is one converged time step = the whole hot path: a1+a2 assemble + eliminate every cell
+(the time step size changes every step, cycling through the sweep, so the matrices really do change), a3 constant
+RHS, a4-a7 fused OCI iterations until max|dphi| < 1e-8 (residual read on the host once every 8 iterations), a8
+advance. value = J x (iterations performed) / device time, summed over the K timed steps.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1 (launched under torchrun, one rank per GPU): independent replicas of the same problem (DESIGN.md "Multi-GPU:
+replicas only"), barrier + max-over-ranks time, value = all ranks' cell-solves / that time, "scaling": "weak".
+--impl reference times the CPU oracle (oracle/, unmodified) on the host cores on bounded samples of the same
+workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import workloads as W  # noqa: E402
+
+SWEEP = [1.0, 1e-1, 1e-2, 1e-3, 1e-4]
+TOL = 1e-8
+CHECK_EVERY = 8
+MAX_ITERS = 4000
+METRIC = "oci_cell_solves_per_s"
+UNIT = "cell-solves/s"
+# dram__bytes_read.sum + dram__bytes_write.sum of one oci_iterate_stream_kernel launch on this workload, from the
+# `ncu --set full` capture summarised in profiles/ (None until captured).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def measured_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            d = json.loads(f.read_text())
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def algorithmic_bytes_per_cell_solve(n: int, G: int) -> int:
+    """A_j^{-1} (8 n^2) + c (8n) + neighbour edge flux (4n) + index/perm (4n) + Psi write (8n) +
+    phi old/new (64 G)."""
+    return 8 * n * n + 24 * n + 64 * G
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for nm, val in zip(names, r[4:8]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference): the ONLY places this file touches oracle/
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_pass(problem, dts):
+    """One converged time step per dt (factor + iterate to convergence + advance) with the unmodified oracle."""
+    from oracle import Oracle, num_threads
+    o = Oracle(problem, dt=dts[0])
+    solves, t0 = 0, time.perf_counter()
+    per_dt = []
+    for dt in dts:
+        t1 = time.perf_counter()
+        o.set_dt(dt)
+        o.factor()
+        it, _ = o.oci_step(tol=TOL, max_iters=MAX_ITERS)
+        per_dt.append({"dt": dt, "iters": int(it), "s": time.perf_counter() - t1})
+        solves += problem.J * it
+    return solves, time.perf_counter() - t0, per_dt, num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    full = W.config5()
+    sample = full.head(args.ref_cells)
+    from oracle import Oracle, num_threads
+    o = Oracle(sample, dt=SWEEP[0])
+    step_s, solves = [], 0
+    for i in range(args.warmup + args.steps):
+        dt = SWEEP[i % len(SWEEP)]
+        t = time.perf_counter()
+        o.set_dt(dt)
+        o.factor()
+        it, _ = o.oci_step(tol=TOL, max_iters=MAX_ITERS)
+        el = time.perf_counter() - t
+        if i >= args.warmup:
+            step_s.append(el)
+            solves += sample.J * it
+    total = sum(step_s)
+    value = solves / total
+    desc = f"first {sample.J} of 65536 cells of config 5, one converged time step per timed step, dt cycling {SWEEP}"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[4] (config 5): G1 S16 n=64 J=65536, dt sweep", "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": num_threads(), "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# GPU arm
+# ---------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2503_00264_b200 import OCISolver
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    p = W.config5()
+    n, J, G = p.n, p.J, p.G
+    oci = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}")
+    si = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}")
+    K, Wm = args.steps, args.warmup
+
+    def oci_step(i, solver=oci):
+        solver.set_dt(SWEEP[i % len(SWEEP)])
+        return solver.step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+
+    # ---- device-resident leg -------------------------------------------------------------------------------
+    for i in range(Wm):
+        oci_step(i)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    per_dt = {dt: {"dt": dt, "oci_iters": [], "oci_ms": [], "factor_ms": [], "iter_kernel_ms": []} for dt in SWEEP}
+    iters_total = launches = 0
+    kernel_ms_total = 0.0
+    barrier()
+    with ClockSampler(local) as clocks:
+        ev0.record()
+        for i in range(Wm, Wm + K):
+            t = time.perf_counter()
+            it, conv, _ = oci_step(i)
+            el = (time.perf_counter() - t) * 1e3   # oci_step is synchronous: host time of the call = its device time + launch gaps
+            kms, ln = oci.last_timing(1)
+            fms, _ = oci.last_timing(0)
+            d = per_dt[SWEEP[i % len(SWEEP)]]
+            d["oci_iters"].append(it); d["oci_ms"].append(el); d["factor_ms"].append(fms); d["iter_kernel_ms"].append(kms)
+            iters_total += it
+            launches += ln
+            kernel_ms_total += kms
+        ev1.record()
+        barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * J * iters_total / (ms_total * 1e-3)
+
+    # ---- SI comparator, same sequence (reported beside, not part of `value`) ----------------------------------
+    for i in range(Wm):
+        si.set_dt(SWEEP[i % len(SWEEP)]); si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+    for i in range(Wm, Wm + K):
+        dt = SWEEP[i % len(SWEEP)]
+        si.set_dt(dt)
+        torch.cuda.synchronize(); t = time.perf_counter()
+        it, conv, _ = si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+        el = (time.perf_counter() - t) * 1e3
+        per_dt[dt].setdefault("si_iters", []).append(it)
+        per_dt[dt].setdefault("si_ms", []).append(el)
+    diff = float((oci.scalar_flux() - si.scalar_flux()).abs().max().item())
+
+    # ---- end-to-end leg: host buffers through oci_step_host, copies inside the timed region ------------------
+    e2e = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}")
+    q_host = torch.from_numpy(np.ascontiguousarray(p.q)).pin_memory()
+    phi_host = torch.empty((J, G, 4), dtype=torch.float64).pin_memory()
+    for i in range(Wm):
+        e2e.set_dt(SWEEP[i % len(SWEEP)])
+        e2e.step_host(0, q_host, phi_host, tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_iters = 0
+    for i in range(Wm, Wm + K):
+        e2e.set_dt(SWEEP[i % len(SWEEP)])
+        it, _, _ = e2e.step_host(0, q_host, phi_host, tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+        e2e_iters += it
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = world * J * e2e_iters / e2e_s
+    nbytes = J * G * 4 * 8
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel (oci_iterate_stream_kernel), from the timed region -----------------------
+    peak, peak_src = measured_peaks()
+    launch_ms = kernel_ms_total / max(iters_total, 1)
+    alg_bytes = algorithmic_bytes_per_cell_solve(n, G) * J
+    achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "oci_iterate_stream_kernel", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": launch_ms,
+                "kernel_share_of_step": kernel_ms_total / ms_total}
+
+    # ---- CPU oracle on the same workload (bounded sample), rank 0, N = 1 only ---------------------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = p.head(args.cpu_cells)
+        solves, secs, cpu_dt, cores = oracle_pass(sample, SWEEP)
+        cpu = {"value": solves / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {sample.J} of {J} cells of config 5, one converged time step at each dt of {SWEEP} "
+                         f"(factor + iterate + advance), {secs:.1f} s",
+               "iters": [d["iters"] for d in cpu_dt]}
+
+    table = []
+    for dt in SWEEP:
+        d = per_dt[dt]
+        if not d["oci_iters"]:
+            continue
+        table.append({"dt": dt, "oci_iters": d["oci_iters"], "si_iters": d.get("si_iters"),
+                      "oci_ms_per_step": statistics.mean(d["oci_ms"]), "oci_factor_ms": statistics.mean(d["factor_ms"]),
+                      "oci_iter_kernel_ms": statistics.mean(d["iter_kernel_ms"]),
+                      "si_ms_per_step": statistics.mean(d["si_ms"]) if d.get("si_ms") else None})
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[4] (config 5): G1 S16 n=64 J=65536, one converged time step per "
+                               "step, dt cycling {1,1e-1,1e-2,1e-3,1e-4}, tol 1e-8, check_every 8",
+                   "J": J, "N": p.N, "G": G, "n": n, "l2_flush": "not needed: 2.1 GB of factors streamed per iteration (17x L2)",
+                   "parallelism": "replicas" if world > 1 else "single"},
+        "clocks": clocks.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "oci_vs_si": table,
+        "max_abs_phi_oci_minus_si": diff,
+        "iterations_total": iters_total,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--cpu-cells", type=int, default=32768, help="cells of the cpu_baseline sample")
+    ap.add_argument("--ref-cells", type=int, default=8192, help="cells per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

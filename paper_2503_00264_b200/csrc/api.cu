@@ -167,8 +167,15 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
     if (rule != OCI_STOP_DPHI_INF && rule != OCI_STOP_PAPER) return -5;
     long long launches = 0;
     int r;
+    if (ctx->opt_refactor_every_step) { // Alg. 2 as printed: `_gesv` in the first iteration of every step
+        if (scheme == 0) ctx->factored = false;
+        else ctx->si_valid = false;
+    }
     if (scheme == 0) {
-        if (!ctx->factored && (r = oci_factor(ctx)) != 0) return r;
+        if (!ctx->factored) {
+            if ((r = oci_factor(ctx)) != 0) return r;
+            launches += ctx->last_launches[0];
+        }
         if ((r = ensure_const_rhs(ctx, &launches)) < 0) return r;
     } else {
         if ((r = ensure_si(ctx, &launches)) < 0) return r;
@@ -177,16 +184,17 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
     const bool want_l2 = rule == OCI_STOP_PAPER;
     ctx->hist_has_l2 = want_l2;
     const int which = scheme == 0 ? 1 : 2;
-    OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     int it = 0, conv_at = 0;
-    double last = INFINITY, e_prev = 0.0;
+    double last = INFINITY, e_prev = 0.0, kernel_ms = 0.0;
     while (it < max_iters && !conv_at) {
         const int k = (max_iters - it < check_every) ? max_iters - it : check_every;
+        OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
         for (int i = 0; i < k; ++i) {
             r = one_iteration(ctx, scheme, it + i, want_l2);
             if (r < 0) return r;
             launches += r;
         }
+        OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
         // the one host round-trip: k residuals, once every k iterations
         double *h_inf = ctx->h_resid, *h_l2 = ctx->h_resid + OCI_RESID_CAP;
         OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_inf + it, ctx->resid_inf + it, sizeof(double) * k, cudaMemcpyDeviceToHost,
@@ -195,6 +203,11 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
             OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_l2 + it, ctx->resid_l2 + it, sizeof(double) * k, cudaMemcpyDeviceToHost,
                                               ctx->stream));
         OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        {
+            float t = 0.f; // device time of this batch of k iterations (kernels only, no flag read)
+            OCI_CUDA_TRY(ctx, cudaEventElapsedTime(&t, ctx->ev0, ctx->ev1));
+            kernel_ms += t;
+        }
         for (int i = 0; i < k && !conv_at; ++i) {
             const int l = it + i;
             if (!want_l2) {
@@ -209,13 +222,13 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
         }
         it += k;
     }
-    OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     ctx->hist_len = it;
-    ctx->last_ms[which] = -1.0;
+    ctx->last_ms[which] = kernel_ms;
     ctx->last_launches[which] = launches;
     if (advance) {
         r = launch_advance(ctx);
         if (r < 0) return r;
+        ctx->last_launches[which] += r;
         ctx->c_valid = false;
     }
     OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
@@ -321,6 +334,7 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     else if (!strcmp(key, "iterate_ctas_per_sm")) ctx->opt_ctas_per_sm = (int)value;
     else if (!strcmp(key, "factor_kernel")) ctx->opt_factor_kernel = (int)value;
     else if (!strcmp(key, "use_graph")) ctx->opt_use_graph = (int)value;
+    else if (!strcmp(key, "refactor_every_step")) ctx->opt_refactor_every_step = (int)value;
     else return -2;
     return 0;
 }
