@@ -282,6 +282,183 @@ __global__ void __launch_bounds__(ITER_THREADS, 1) oci_iterate_stream_kernel(con
 }
 
 // ============================================================================================================
+// Warp-per-cell streaming kernel (n = 64, 128, 256): the production path for the large configurations.
+// ============================================================================================================
+// Every consumer warp owns one cell at a time: lane l holds the rows {64 q + 2 l, 64 q + 2 l + 1}, q < RPL/2, of
+// x = A^{-1} b in registers, so a column of the inverse is RPL/2 conflict-free 16-byte shared-memory loads per
+// lane and the product needs no cross-warp reduction, no CTA-wide barrier and no shuffles. A cell spans
+// NCH = n / CW chunks (column panels of CW = 2048 / n columns, 16 KB each); the producer interleaves the chunks
+// of WC consecutive cells (one per consumer warp) so that all warps stream concurrently. The per-cell prologue (b = c + incident) and epilogue (Psi store, phi, residual)
+// are warp-local as well, so the only synchronisation is the mbarrier handshake with the bulk-copy engine.
+// Every consumer warp has its OWN ring of `spw` stages (single producer, single consumer per mbarrier): a shared
+// ring would let a warp test a stage's parity one phase early and read a chunk that has not landed.
+constexpr int WPC_WARPS = 4;                      // consumer warps (one per SM sub-partition)
+constexpr int WPC_THREADS = (WPC_WARPS + 1) * 32;
+constexpr int WPC_VEC_SLOTS = 2;
+constexpr int WPC_CHUNK = 2048;                   // doubles per chunk (16 KB)
+constexpr int WPC_MAX_STAGES = 16;                // WPC_WARPS x stages per warp
+
+template <int RPL, bool WANT_L2>
+__global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const IterParams P)
+{
+    constexpr int n = 32 * RPL;
+    constexpr int CW = WPC_CHUNK / n;   // columns per chunk
+    constexpr int NCH = n / CW;         // chunks per cell
+    constexpr int HQ = RPL / 2;         // 16-byte loads per lane per column
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int N = P.N, G = P.G, J = P.J, spw = P.stages; // stages per consumer warp
+    constexpr int vec_c = WPC_WARPS * n, vec_nb = (WPC_WARPS + 2) * n;
+
+    uint64_t *mat_full = reinterpret_cast<uint64_t *>(smem_raw);
+    uint64_t *mat_empty = mat_full + WPC_MAX_STAGES;
+    uint64_t *vec_full = mat_empty + WPC_MAX_STAGES;
+    uint64_t *vec_empty = vec_full + WPC_VEC_SLOTS;
+    double *mu_s = reinterpret_cast<double *>(vec_empty + WPC_VEC_SLOTS); // [N]
+    double *w_s = mu_s + N;                                              // [N]
+    size_t off = (size_t)((unsigned char *)(w_s + N) - smem_raw);
+    off = (off + 127) & ~(size_t)127;
+    double *vec = reinterpret_cast<double *>(smem_raw + off);            // WPC_VEC_SLOTS x (vec_c + vec_nb)
+    off += (size_t)WPC_VEC_SLOTS * (vec_c + vec_nb) * sizeof(double);
+    off = (off + 127) & ~(size_t)127;
+    double *mat = reinterpret_cast<double *>(smem_raw + off);            // [WPC_WARPS][spw] x WPC_CHUNK
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int s = 0; s < WPC_WARPS * spw; ++s) { mbar_init(&mat_full[s], 1); mbar_init(&mat_empty[s], 1); }
+        for (int s = 0; s < WPC_VEC_SLOTS; ++s) { mbar_init(&vec_full[s], 1); mbar_init(&vec_empty[s], WPC_WARPS); }
+        fence_mbar_init();
+    }
+    for (int i = tid; i < N; i += WPC_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    __syncthreads();
+
+    // balanced contiguous split of the cells over the CTAs
+    const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
+    const int cell1 = (int)(((long long)J * (blockIdx.x + 1)) / gridDim.x);
+
+    if (warp == WPC_WARPS) {
+        // ===================== producer ==================================================================
+        if (lane == 0) {
+            int vs = 0;
+            uint32_t vph = 0;
+            unsigned it = 0; // chunk round: every warp with a cell gets one chunk per round
+            for (int gb = cell0; gb < cell1; gb += WPC_WARPS) {
+                const int nv = min(WPC_WARPS, cell1 - gb);
+                mbar_wait(&vec_empty[vs], vph ^ 1);
+                {
+                    double *cs = vec + (size_t)vs * (vec_c + vec_nb);
+                    double *nb = cs + vec_c;
+                    const int lo = max(gb - 1, 0), hi = min(gb + nv, J - 1);
+                    const uint32_t bytes_c = (uint32_t)(nv * n * sizeof(double));
+                    const uint32_t bytes_nb = (uint32_t)((hi - lo + 1) * n * sizeof(double));
+                    mbar_arrive_expect_tx(&vec_full[vs], bytes_c + bytes_nb);
+                    bulk_g2s(cs, P.c + (size_t)gb * n, bytes_c, &vec_full[vs]);
+                    bulk_g2s(nb + (size_t)(lo - (gb - 1)) * n, P.psi_old + (size_t)lo * n, bytes_nb, &vec_full[vs]);
+                }
+                if (++vs == WPC_VEC_SLOTS) { vs = 0; vph ^= 1; }
+                for (int k = 0; k < NCH; ++k, ++it) {
+                    const int slot = it % spw;
+                    const uint32_t ph = (it / spw) & 1;
+                    for (int w = 0; w < nv; ++w) {
+                        const int st = w * spw + slot;
+                        mbar_wait(&mat_empty[st], ph ^ 1);
+                        mbar_arrive_expect_tx(&mat_full[st], WPC_CHUNK * sizeof(double));
+                        bulk_g2s(mat + (size_t)st * WPC_CHUNK, P.Minv + (size_t)(gb + w) * n * n + (size_t)k * CW * n,
+                                 WPC_CHUNK * sizeof(double), &mat_full[st]);
+                    }
+                }
+            }
+        }
+        return;
+    }
+
+    // ========================= consumer warps ===============================================================
+    int vs = 0;
+    uint32_t vph = 0;
+    unsigned it = 0;
+    double rmax = 0.0, l2 = 0.0;
+    for (int gb = cell0; gb < cell1; gb += WPC_WARPS) {
+        const int nv = min(WPC_WARPS, cell1 - gb);
+        double *cs = vec + (size_t)vs * (vec_c + vec_nb);
+        const double *nb = cs + vec_c;
+        mbar_wait(&vec_full[vs], vph);
+        if (warp < nv) {
+            const int j = gb + warp;
+            double *bs = cs + warp * n;                 // this warp's c_j, turned into b_j in place (a4)
+            const double *own = nb + (warp + 1) * n;     // Psi^(l) of this cell
+            for (int i = lane; i < n; i += 32) bs[i] += incident_term(P, nb, gb, j, i, mu_s);
+            __syncwarp();
+
+            // ---- a5: x = A^{-1} b
+            double acc[2][RPL];
+#pragma unroll
+            for (int r = 0; r < RPL; ++r) { acc[0][r] = 0.0; acc[1][r] = 0.0; }
+            for (int k = 0; k < NCH; ++k) {
+                const unsigned r = it + (unsigned)k;
+                const int st = warp * spw + (int)(r % spw);
+                mbar_wait(&mat_full[st], (r / spw) & 1);
+                const double2 *Mp = reinterpret_cast<const double2 *>(mat + (size_t)st * WPC_CHUNK) + lane;
+                const double2 *bp = reinterpret_cast<const double2 *>(bs + k * CW);
+#pragma unroll 4
+                for (int cc = 0; cc < CW; cc += 2) {
+                    const double2 bv = bp[cc >> 1];
+#pragma unroll
+                    for (int q = 0; q < HQ; ++q) {
+                        const double2 m0 = Mp[(cc * n) / 2 + q * 32];
+                        const double2 m1 = Mp[((cc + 1) * n) / 2 + q * 32];
+                        acc[0][2 * q] = fma(m0.x, bv.x, acc[0][2 * q]);
+                        acc[0][2 * q + 1] = fma(m0.y, bv.x, acc[0][2 * q + 1]);
+                        acc[1][2 * q] = fma(m1.x, bv.y, acc[1][2 * q]);
+                        acc[1][2 * q + 1] = fma(m1.y, bv.y, acc[1][2 * q + 1]);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&mat_empty[st]);
+            }
+
+            // ---- Psi^(l+1): rows 64 q + 2 lane, + 1; kept in shared memory (over b) for the phi reduction
+            double2 *xs2 = reinterpret_cast<double2 *>(bs);
+            double2 *out2 = reinterpret_cast<double2 *>(P.psi_new + (size_t)j * n);
+#pragma unroll
+            for (int q = 0; q < HQ; ++q) {
+                const double2 x = make_double2(acc[0][2 * q] + acc[1][2 * q], acc[0][2 * q + 1] + acc[1][2 * q + 1]);
+                if (WANT_L2) {
+                    const double2 o = reinterpret_cast<const double2 *>(own)[q * 32 + lane];
+                    const double d0 = x.x - o.x, d1 = x.y - o.y;
+                    l2 = fma(d0, d0, l2);
+                    l2 = fma(d1, d1, l2);
+                }
+                xs2[q * 32 + lane] = x;
+                out2[q * 32 + lane] = x;
+            }
+            __syncwarp();
+
+            // ---- a6 + a7: phi of the new and of the previous iterate, residual
+            for (int e = lane; e < G * 4; e += 32) {
+                const int p = e & 3, g = e >> 2;
+                const double *xn = bs + g * N * 4 + p;
+                const double *xo = own + g * N * 4 + p;
+                double sn = 0.0, so = 0.0;
+                for (int m = 0; m < N; ++m) { sn = fma(w_s[m], xn[m * 4], sn); so = fma(w_s[m], xo[m * 4], so); }
+                P.phi[(size_t)j * G * 4 + e] = sn;
+                const double d = fabs(sn - so);
+                rmax = (d > rmax || !(d == d)) ? d : rmax;
+            }
+        }
+        it += NCH;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&vec_empty[vs]);
+        if (++vs == WPC_VEC_SLOTS) { vs = 0; vph ^= 1; }
+    }
+    rmax = warp_max(rmax);
+    if (lane == 0 && cell1 > cell0) atomicMax(P.resid_inf, resid_bits(rmax));
+    if (WANT_L2) {
+        l2 = warp_sum(l2);
+        if (lane == 0 && cell1 > cell0) atomicAdd(P.resid_l2, l2);
+    }
+}
+
+// ============================================================================================================
 // Plain kernel: one CTA per cell, loads straight from global memory. Used for cross-checking the pipelined
 // kernel and selectable with oci_set_option("iterate_kernel", 0).
 // ============================================================================================================
@@ -449,7 +626,35 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2)
     P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
     P.resid_inf = ctx->resid_inf + hist_slot;
     P.resid_l2 = ctx->resid_l2 + hist_slot;
-    if (ctx->opt_iterate_kernel == 0 || ctx->n > CONSUMERS) {
+    const bool wpc_ok = ctx->n == 64 || ctx->n == 128 || ctx->n == 256;
+    if (ctx->opt_iterate_kernel == 1 && wpc_ok) {
+        const int n = ctx->n;
+        const size_t fixed = (size_t)(2 * WPC_MAX_STAGES + 2 * WPC_VEC_SLOTS) * 8 + (size_t)(2 * ctx->N) * 8 + 256 +
+                             (size_t)WPC_VEC_SLOTS * ((2 * WPC_WARPS + 2) * n) * 8 + 128;
+        int stages = (int)(((size_t)ctx->max_smem_optin - fixed) / ((size_t)WPC_CHUNK * 8 * WPC_WARPS)); // per warp
+        if (stages > WPC_MAX_STAGES / WPC_WARPS) stages = WPC_MAX_STAGES / WPC_WARPS;
+        if (ctx->opt_stages > 0 && ctx->opt_stages < stages) stages = ctx->opt_stages;
+        if (stages < 1) stages = 1;
+        const size_t smem = fixed + (size_t)stages * WPC_WARPS * WPC_CHUNK * 8;
+        P.cpb = 1; P.S = 1; P.cw = WPC_CHUNK / n; P.nch = n / P.cw; P.n_items = ctx->J; P.stages = stages;
+        P.chunk_doubles = WPC_CHUNK;
+        int grid = ctx->num_sms;
+        if (grid > (ctx->J + WPC_WARPS - 1) / WPC_WARPS) grid = (ctx->J + WPC_WARPS - 1) / WPC_WARPS;
+#define OCI_WPC_LAUNCH(RPL_, L2_)                                                                                  \
+    do {                                                                                                           \
+        static size_t attr = 0;                                                                                    \
+        if (attr < smem) {                                                                                         \
+            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(oci_iterate_wpc_kernel<RPL_, L2_>,                               \
+                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+            attr = smem;                                                                                           \
+        }                                                                                                          \
+        oci_iterate_wpc_kernel<RPL_, L2_><<<grid, WPC_THREADS, smem, ctx->stream>>>(P);                             \
+    } while (0)
+        if (n == 64) { if (want_l2) OCI_WPC_LAUNCH(2, true); else OCI_WPC_LAUNCH(2, false); }
+        else if (n == 128) { if (want_l2) OCI_WPC_LAUNCH(4, true); else OCI_WPC_LAUNCH(4, false); }
+        else { if (want_l2) OCI_WPC_LAUNCH(8, true); else OCI_WPC_LAUNCH(8, false); }
+#undef OCI_WPC_LAUNCH
+    } else if (ctx->opt_iterate_kernel == 0 || ctx->n > CONSUMERS) {
         P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
         const size_t smem = (size_t)(5 * ctx->n + 2 * ctx->N) * sizeof(double);
         int grid = ctx->num_sms * 8;
