@@ -7,7 +7,9 @@
 // pivots `_gesv` takes in Alg. 2 -- carried through to the inverse (Gauss-Jordan, in
 // place, implicit row exchange), because the iterate kernel streams A_j^{-1}.
 #include "common.cuh"
+#include <cooperative_groups.h>
 #include <limits.h>
+#include <string.h>
 
 namespace {
 
@@ -126,6 +128,264 @@ factor_gj_kernel(ProblemView P, double *__restrict__ Minv, double *__restrict__ 
     }
 }
 
+// ============================================================================================================
+// Register-tiled, panel-blocked Gauss-Jordan for n = 64 NQ (NQ = 1..4): the production a1 + a2 kernel.
+// ============================================================================================================
+// One cluster of NQ CTAs per cell; CTA q owns the columns [64 q, 64 q + 64), warp w of it the 8-column tile
+// [64 q + 8 w, +8), lane l the rows {64 s + 2 l, 64 s + 2 l + 1}, s < NQ: the whole working matrix W lives in
+// registers (TR x 8 = n / 4 doubles per thread) and is never written anywhere un-eliminated.
+//
+// In-place Gauss-Jordan with implicit row exchange, blocked by panels of NB = 8 columns K = {k_0..k_7}:
+//   phase P  the warp that owns the panel runs the 8 elimination steps on its n x 8 tile alone (warp-level
+//            operations only): pivot row r_b = first row of maximal |W[i][k_b]| among the unused rows (three
+//            redux.sync on the bit pattern), pivot row broadcast by shuffles, W[r][:] /= p, W[i][:] -= f_i W[r][:].
+//            Afterwards column k_b of the tile holds T e_{r_b}, T = the product of the 8 elementary matrices.
+//   phase U  T differs from I only in the columns R = {r_b}, so every other column c becomes
+//            W[:, c] + Z W_old[R, c] with Z = T[:, R] - I[:, R]  (n x 8). The owner publishes Z and R to every
+//            CTA of the cluster (distributed shared memory), each thread that holds a pivot row publishes its
+//            old 8 entries of it (Rrow), and every warp but the owner applies the rank-8 update to its tile.
+// Two barriers per 8 pivots (one cluster-wide, one CTA-wide); Z / Rrow / R are double-buffered so that no third
+// barrier is needed. At the end W[i][j] = A^{-1}[rhoinv[i]][rho[j]] (rho[k] = pivot row of step k).
+namespace cg = cooperative_groups;
+
+constexpr int FR_THREADS = 256;
+constexpr int FR_NB = 8;
+
+template <int NQ> struct FrShared {
+    double Z[2][FR_NB][64 * NQ];          // [buf][b][row]
+    double Rrow[2][FR_NB][64];            // [buf][b][local column]
+    double bcast[FR_THREADS / 32][2][10]; // per warp: pivot row (8) + 1/pivot of a panel step, two slots
+    int R[2][FR_NB];                      // pivot rows of the panel
+    int sing[2];                          // panel met a zero / non-finite pivot
+    int rho[64 * NQ], rhoinv[64 * NQ];
+};
+
+template <int NQ>
+__global__ void __launch_bounds__(FR_THREADS, NQ == 1 ? 3 : (NQ == 2 ? 2 : 1))
+factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
+{
+    constexpr int n = 64 * NQ, TR = 2 * NQ, NPANEL = n / FR_NB;
+    __shared__ __align__(16) FrShared<NQ> sh;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int q = NQ == 1 ? 0 : (int)cluster.block_rank();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int n_clusters = gridDim.x / NQ, cluster_id = blockIdx.x / NQ;
+    const int N = P.N, G = P.G;
+    const unsigned FULL = 0xffffffffu;
+    unsigned gp = 0; // running panel counter: selects the shared-memory buffer
+
+    auto cluster_barrier = [&]() {
+        if (NQ == 1) __syncthreads();
+        else cluster.sync();
+    };
+
+    for (int cell = cluster_id; cell < P.J; cell += n_clusters) {
+        // ---- a1: assemble the tile, bit-identical to a_entry() (same operations in the same order)
+        double a[TR][8];
+        {
+            const double dx = P.dx[cell];
+            const int p0 = (lane & 1) * 2; // p of row 64 s + 2 lane
+            double Kw[2][NQ], wq[2];       // per column half: transfer entry (per row group) and weight
+            int bmc[2];
+#pragma unroll
+            for (int hc = 0; hc < 2; ++hc) {
+                bmc[hc] = 16 * q + 2 * w + hc;
+                wq[hc] = P.w[bmc[hc] % N];
+            }
+#pragma unroll
+            for (int s = 0; s < NQ; ++s) {
+                const int bm = 16 * s + (lane >> 1), m = bm % N, g = bm / N;
+                const double sig = P.sigma_t[(size_t)cell * G + g], mu = P.mu[m];
+                const double av = __dmul_rn(__dadd_rn(fabs(mu), __dmul_rn(dx, sig)), 0.5);
+                const double gam = __ddiv_rn(dx, __dmul_rn(P.v[g], P.dt));
+                const double h = __dmul_rn(mu, 0.5), hg = __dmul_rn(gam, 0.5), ga = __dadd_rn(gam, av);
+#pragma unroll
+                for (int hc = 0; hc < 2; ++hc) {
+                    const double K = P.transfer[((size_t)cell * G + g) * G + bmc[hc] / N];
+                    Kw[hc][s] = __dmul_rn(__dmul_rn(__dmul_rn(dx, K), 0.25), wq[hc]);
+                }
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int p = p0 + e;
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const int pp = c & 3, hc = c >> 2;
+                        double val = 0.0;
+                        if (bm == bmc[hc]) { // Eq. 8b
+                            const int d = pp - p;
+                            if (d == 0) val = p < 2 ? av : ga;
+                            else if (p == 0 && pp == 1) val = h;
+                            else if (p == 1 && pp == 0) val = -h;
+                            else if (p == 2 && pp == 3) val = h;
+                            else if (p == 3 && pp == 2) val = -h;
+                            else if (d == 2) val = hg;       // (0,2), (1,3)
+                            else if (d == -2) val = -gam;    // (2,0), (3,1)
+                        }
+                        if (p == pp) val = __dsub_rn(val, Kw[hc][s]);
+                        a[2 * s + e][c] = val;
+                    }
+                }
+            }
+        }
+        unsigned usedmask = 0;
+        bool singular = false;
+
+        for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
+            const int buf = gp & 1;
+            const bool owner = (pnl >> 3) == q && (pnl & 7) == w;
+            if (owner) {
+                // ================= phase P: eliminate the n x 8 panel inside this warp =====================
+                int Rl[FR_NB];
+                bool bad = false;
+                unsigned um = usedmask;
+                double *bc = &sh.bcast[w][0][0];
+#pragma unroll
+                for (int b = 0; b < FR_NB; ++b) {
+                    // local candidate: first row of maximal |entry| among this lane's unused rows
+                    unsigned long long bk = 0ull;
+                    int brow = INT_MAX;
+                    double bval = 1.0;
+#pragma unroll
+                    for (int rr = 0; rr < TR; ++rr) {
+                        const unsigned long long key = (unsigned long long)__double_as_longlong(fabs(a[rr][b]));
+                        if (!((um >> rr) & 1u) && (brow == INT_MAX || key > bk)) {
+                            bk = key;
+                            brow = 64 * (rr >> 1) + 2 * lane + (rr & 1);
+                            bval = a[rr][b];
+                        }
+                    }
+                    const double linv = 1.0 / bval; // of the lane's own candidate: overlaps the arg-max below
+                    const unsigned khi = (unsigned)(bk >> 32), klo = (unsigned)bk;
+                    const unsigned mhi = __reduce_max_sync(FULL, brow == INT_MAX ? 0u : khi);
+                    const bool c1 = brow != INT_MAX && khi == mhi;
+                    const unsigned mlo = __reduce_max_sync(FULL, c1 ? klo : 0u);
+                    const bool c2 = c1 && klo == mlo;
+                    const int r = __reduce_min_sync(FULL, c2 ? brow : INT_MAX);
+                    const unsigned long long mk = ((unsigned long long)mhi << 32) | mlo;
+                    if (mk == 0ull || mk >= 0x7ff0000000000000ull) bad = true; // zero, inf or NaN pivot
+                    Rl[b] = r;
+                    const int lane_r = (r & 63) >> 1, rr_r = 2 * (r >> 6) + (r & 1); // warp-uniform
+                    const bool mine = lane == lane_r;
+                    // pivot row and 1/pivot through a per-warp shared-memory slot (two slots alternate)
+                    double *slot = bc + (b & 1) * 10;
+#pragma unroll
+                    for (int rr = 0; rr < TR; ++rr)
+                        if (rr == rr_r && mine) {
+#pragma unroll
+                            for (int c = 0; c < 4; ++c)
+                                reinterpret_cast<double2 *>(slot)[c] = make_double2(a[rr][2 * c], a[rr][2 * c + 1]);
+                            slot[8] = linv;
+                        }
+                    __syncwarp();
+                    double sp[8];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const double2 t = reinterpret_cast<const double2 *>(slot)[c];
+                        sp[2 * c] = t.x;
+                        sp[2 * c + 1] = t.y;
+                    }
+                    const double inv = slot[8];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) sp[c] = (c == b) ? inv : sp[c] * inv;
+#pragma unroll
+                    for (int rr = 0; rr < TR; ++rr) {
+                        const double f = a[rr][b];
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) a[rr][c] = (c == b) ? -f * inv : fma(-f, sp[c], a[rr][c]);
+                    }
+#pragma unroll
+                    for (int rr = 0; rr < TR; ++rr)
+                        if (rr == rr_r && mine) {
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) a[rr][c] = sp[c];
+                        }
+                    if (mine) um |= 1u << rr_r;
+                }
+                // ---- publish Z = T[:, R] - I[:, R], R and the singular flag to every CTA of the cluster
+#pragma unroll
+                for (int t = 0; t < NQ; ++t) {
+                    FrShared<NQ> *dst = NQ == 1 ? &sh : cluster.map_shared_rank(&sh, t);
+#pragma unroll
+                    for (int b = 0; b < FR_NB; ++b) {
+#pragma unroll
+                        for (int s = 0; s < NQ; ++s) {
+                            const int row0 = 64 * s + 2 * lane;
+                            double2 z;
+                            z.x = a[2 * s][b] - (Rl[b] == row0 ? 1.0 : 0.0);
+                            z.y = a[2 * s + 1][b] - (Rl[b] == row0 + 1 ? 1.0 : 0.0);
+                            *reinterpret_cast<double2 *>(&dst->Z[buf][b][row0]) = z;
+                        }
+                        if (lane == b) dst->R[buf][b] = Rl[b];
+                    }
+                    if (lane == 0) dst->sing[buf] = bad ? 1 : 0;
+                }
+            }
+            cluster_barrier(); // B1: Z, R, sing of this panel visible everywhere
+
+            if (sh.sing[buf]) { singular = true; ++gp; break; } // uniform across the cluster
+            // ---- every thread: note the pivot rows; holders publish the OLD entries of their pivot rows
+#pragma unroll
+            for (int b = 0; b < FR_NB; ++b) {
+                const int r = sh.R[buf][b];
+                const int lane_r = (r & 63) >> 1, rr_r = 2 * (r >> 6) + (r & 1);
+                if (lane == lane_r) {
+                    usedmask |= 1u << rr_r;
+                    if (!owner) {
+                        double2 *dst = reinterpret_cast<double2 *>(&sh.Rrow[buf][b][8 * w]);
+#pragma unroll
+                        for (int rr = 0; rr < TR; ++rr)
+                            if (rr == rr_r) {
+#pragma unroll
+                                for (int c = 0; c < 4; ++c) dst[c] = make_double2(a[rr][2 * c], a[rr][2 * c + 1]);
+                            }
+                    }
+                }
+                if (w == 0 && lane == b) { sh.rho[FR_NB * pnl + b] = r; sh.rhoinv[r] = FR_NB * pnl + b; }
+            }
+            __syncthreads(); // B2: Rrow of this CTA complete
+
+            if (!owner) {
+                // ================= phase U: rank-8 update of this thread's TR x 8 tile =======================
+#pragma unroll
+                for (int b = 0; b < FR_NB; ++b) {
+                    double rv[8];
+                    const double2 *src = reinterpret_cast<const double2 *>(&sh.Rrow[buf][b][8 * w]);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) { const double2 t = src[c]; rv[2 * c] = t.x; rv[2 * c + 1] = t.y; }
+#pragma unroll
+                    for (int s = 0; s < NQ; ++s) {
+                        const double2 z = *reinterpret_cast<const double2 *>(&sh.Z[buf][b][64 * s + 2 * lane]);
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) {
+                            a[2 * s][c] = fma(z.x, rv[c], a[2 * s][c]);
+                            a[2 * s + 1][c] = fma(z.y, rv[c], a[2 * s + 1][c]);
+                        }
+                    }
+                }
+            }
+        }
+
+        double *out = Minv + (size_t)cell * n * n;
+        if (singular) {
+            if (q == 0 && threadIdx.x == 0) atomicMin(info, cell + 1);
+            // leave a NaN-free but meaningless block behind: zero this CTA's share
+            for (int e = threadIdx.x; e < 64 * n; e += FR_THREADS) out[(size_t)64 * q * n + e] = 0.0;
+            cluster_barrier(); // nobody may start the next cell's panels while a peer still reads this one's flags
+            continue;
+        }
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]
+        int ro[TR];
+#pragma unroll
+        for (int rr = 0; rr < TR; ++rr) ro[rr] = sh.rhoinv[64 * (rr >> 1) + 2 * lane + (rr & 1)];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            double *col = out + (size_t)sh.rho[64 * q + 8 * w + c] * n;
+#pragma unroll
+            for (int rr = 0; rr < TR; ++rr) col[ro[rr]] = a[rr][c];
+        }
+    }
+}
+
 __global__ void assemble_one_kernel(ProblemView P, int cell, double *__restrict__ A)
 {
     const int n = P.n;
@@ -153,11 +413,49 @@ size_t factor_scratch_bytes(int n, int num_sms, int max_smem_optin)
     return one * (size_t)num_sms * 4;
 }
 
+template <int NQ> static int launch_factor_reg(oci_ctx *ctx, const ProblemView &P)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.blockDim = dim3(FR_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = NQ;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = NQ > 1 ? 1 : 0;
+    int n_clusters = 0;
+    if (NQ > 1) {
+        cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_reg_kernel<NQ>, &cfg));
+    } else {
+        int per_sm = 0;
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_reg_kernel<NQ>, FR_THREADS, 0));
+        n_clusters = per_sm * ctx->num_sms;
+    }
+    if (n_clusters < 1) n_clusters = 1;
+    if (n_clusters > ctx->J) n_clusters = ctx->J;
+    cfg.gridDim = dim3(NQ * n_clusters, 1, 1);
+    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_reg_kernel<NQ>, P, ctx->Minv, ctx->info));
+    return 1;
+}
+
 int launch_factor(oci_ctx *ctx)
 {
     const int n = ctx->n;
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream)); // 0x7f7f7f7f = "none"
+    if (ctx->opt_factor_kernel == 1 && n % 64 == 0 && n <= 256) {
+        switch (n / 64) {
+        case 1: return launch_factor_reg<1>(ctx, P);
+        case 2: return launch_factor_reg<2>(ctx, P);
+        case 3: return launch_factor_reg<3>(ctx, P);
+        default: return launch_factor_reg<4>(ctx, P);
+        }
+    }
     const bool global_w = factor_smem_bytes(n, false) > (size_t)ctx->max_smem_optin;
     const size_t smem = factor_smem_bytes(n, global_w);
     int grid;
