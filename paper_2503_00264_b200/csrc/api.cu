@@ -88,11 +88,13 @@ size_t carve(oci_ctx *c, unsigned char *base, int J, int N, int G, int num_sms, 
     t->si_in = cv.take<double>((size_t)J * GN * 2);
     t->resid_inf = cv.take<unsigned long long>(OCI_RESID_CAP);
     t->resid_l2 = cv.take<double>(OCI_RESID_CAP);
+    t->ctrl = cv.take<int>(4);
     return cv.off;
 }
 
 int reset_history(oci_ctx *ctx)
 {
+    OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->ctrl, 0, sizeof(int) * 4, ctx->stream));
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->resid_inf, 0, sizeof(unsigned long long) * OCI_RESID_CAP, ctx->stream));
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->resid_l2, 0, sizeof(double) * OCI_RESID_CAP, ctx->stream));
     ctx->hist_len = 0;
@@ -123,9 +125,20 @@ int ensure_si(oci_ctx *ctx, long long *launches)
 }
 
 // scheme 0 = OCI, 1 = SI
-int one_iteration(oci_ctx *ctx, int scheme, int slot, bool want_l2)
+int one_iteration(oci_ctx *ctx, int scheme, int slot, bool want_l2, bool check_prev)
 {
-    return scheme == 0 ? launch_oci_iteration(ctx, slot, want_l2) : launch_si_iteration(ctx, slot, want_l2);
+    return scheme == 0 ? launch_oci_iteration(ctx, slot, want_l2, check_prev)
+                       : launch_si_iteration(ctx, slot, want_l2, check_prev);
+}
+
+// The stop rule on the host: slot l of the history h (rule 0: max|dphi|; rule 1: sums of squares). Same arithmetic,
+// operation by operation, as stop_reached() on the device.
+bool rule_holds(int rule, double tol, const double *h_inf, const double *h_l2, int l)
+{
+    if (rule == OCI_STOP_DPHI_INF) return h_inf[l] < tol;
+    if (l < 1) return false;
+    const double e = sqrt(h_l2[l]), ep = sqrt(h_l2[l - 1]);
+    return e < tol * (1.0 - e / ep);
 }
 
 int iterate_impl(oci_ctx *ctx, int scheme, int n_iters)
@@ -146,7 +159,7 @@ int iterate_impl(oci_ctx *ctx, int scheme, int n_iters)
     const int which = scheme == 0 ? 1 : 2;
     OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     for (int i = 0; i < n_iters; ++i) {
-        r = one_iteration(ctx, scheme, ctx->hist_len + i, false);
+        r = one_iteration(ctx, scheme, ctx->hist_len + i, false, false);
         if (r < 0) return r;
         launches += r;
     }
@@ -185,42 +198,42 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
     ctx->hist_has_l2 = want_l2;
     const int which = scheme == 0 ? 1 : 2;
     int it = 0, conv_at = 0;
-    double last = INFINITY, e_prev = 0.0, kernel_ms = 0.0;
+    double last = INFINITY, kernel_ms = 0.0;
+    ctx->stop_tol = tol;
+    ctx->stop_rule = rule;
+    double *h_inf = ctx->h_resid, *h_l2 = ctx->h_resid + OCI_RESID_CAP;
+    int *h_exec = reinterpret_cast<int *>(ctx->h_resid + 2 * OCI_RESID_CAP);
     while (it < max_iters && !conv_at) {
         const int k = (max_iters - it < check_every) ? max_iters - it : check_every;
         OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
         for (int i = 0; i < k; ++i) {
-            r = one_iteration(ctx, scheme, it + i, want_l2);
+            // slot it + i > it looks at slot it + i - 1 on the device and skips itself once the rule held
+            r = one_iteration(ctx, scheme, it + i, want_l2, i > 0);
             if (r < 0) return r;
             launches += r;
         }
         OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
-        // the one host round-trip: k residuals, once every k iterations
-        double *h_inf = ctx->h_resid, *h_l2 = ctx->h_resid + OCI_RESID_CAP;
+        // the one host round-trip: k residuals + the executed-iterations counter, once every k iterations
         OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_inf + it, ctx->resid_inf + it, sizeof(double) * k, cudaMemcpyDeviceToHost,
                                           ctx->stream));
         if (want_l2)
             OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_l2 + it, ctx->resid_l2 + it, sizeof(double) * k, cudaMemcpyDeviceToHost,
                                               ctx->stream));
+        OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_exec, ctx->ctrl, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
         {
-            float t = 0.f; // device time of this batch of k iterations (kernels only, no flag read)
+            float t = 0.f; // device time of this batch of k launches (kernels only, no flag read)
             OCI_CUDA_TRY(ctx, cudaEventElapsedTime(&t, ctx->ev0, ctx->ev1));
             kernel_ms += t;
         }
-        for (int i = 0; i < k && !conv_at; ++i) {
-            const int l = it + i;
-            if (!want_l2) {
-                last = h_inf[l];
-                if (last < tol) conv_at = l + 1;
-            } else {
-                const double e = sqrt(h_l2[l]);
-                last = e;
-                if (l >= 1 && e < tol * (1.0 - e / e_prev)) conv_at = l + 1;
-                e_prev = e;
-            }
-        }
-        it += k;
+        const int executed = *h_exec; // iterations of this step that really ran (<= it + k)
+        if (executed < it + 1 || executed > it + k) return OCI_E_STATE;
+        if (scheme == 0 && ((it + k - executed) & 1)) ctx->cur ^= 1; // skipped launches did not swap the Jacobi buffers
+        const int l = executed - 1;
+        last = want_l2 ? sqrt(h_l2[l]) : h_inf[l];
+        if (executed < it + k) conv_at = executed;                       // the device saw the rule hold at slot l
+        else if (rule_holds(rule, tol, h_inf, h_l2, l)) conv_at = executed; // last slot of the batch: tested here
+        it = executed;
     }
     ctx->hist_len = it;
     ctx->last_ms[which] = kernel_ms;
@@ -238,6 +251,20 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
 }
 
 } // namespace
+
+StopCheck make_stop(const oci_ctx *ctx, int slot, bool check_prev)
+{
+    StopCheck s;
+    const bool chk = check_prev && slot >= 1;
+    s.prev_inf = chk ? ctx->resid_inf + slot - 1 : nullptr;
+    s.prev_l2 = chk ? ctx->resid_l2 + slot - 1 : nullptr;
+    s.prev2_l2 = (chk && slot >= 2) ? ctx->resid_l2 + slot - 2 : nullptr;
+    s.tol = ctx->stop_tol;
+    s.rule = ctx->stop_rule;
+    s.slot = slot;
+    s.executed = ctx->ctrl;
+    return s;
+}
 
 extern "C" {
 
@@ -270,7 +297,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     device_limits(&ctx->num_sms, &ctx->max_smem_optin);
     const size_t need = carve(ctx, (unsigned char *)workspace_dev, p->J, p->N, p->G, ctx->num_sms, ctx->max_smem_optin);
     if (need > workspace_bytes) return fail(OCI_E_WORKSPACE);
-    if (cudaHostAlloc((void **)&ctx->h_resid, sizeof(double) * 2 * OCI_RESID_CAP, cudaHostAllocDefault) != cudaSuccess)
+    if (cudaHostAlloc((void **)&ctx->h_resid, sizeof(double) * (2 * OCI_RESID_CAP + 2), cudaHostAllocDefault) != cudaSuccess)
         return fail(OCI_E_CUDA);
     if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) return fail(OCI_E_CUDA);
     cudaStream_t s = ctx->stream;
@@ -295,6 +322,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     ZERO(ctx->phi, sizeof(double) * J * G * 4);
     ZERO(ctx->resid_inf, sizeof(double) * OCI_RESID_CAP);
     ZERO(ctx->resid_l2, sizeof(double) * OCI_RESID_CAP);
+    ZERO(ctx->ctrl, sizeof(int) * 4);
 #undef ZERO
     if (cudaStreamSynchronize(s) != cudaSuccess) return fail(OCI_E_CUDA);
     *out = ctx;

@@ -54,6 +54,10 @@ struct oci_ctx {
     int hist_len;                  // iterations recorded since the history was last reset
     int hist_has_l2;
 
+    int *ctrl;                     // [4] ctrl[0] = iterations of the current step that really ran (device-side stop)
+    double stop_tol;               // stop rule the device applies between the iterations of one batch
+    int stop_rule;
+
     bool factored, c_valid, si_valid, phi_valid;
     // options
     int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph, opt_refactor_every_step;
@@ -73,7 +77,22 @@ struct ProblemView {
     const double *dx, *sigma_t, *transfer, *v, *mu, *w;
 };
 
+// Device-side stop: iteration `slot` of a batch first looks at the residual slot - 1, which
+// is complete because launches are stream-ordered, and returns at once if the stop rule held there. Skipped slots
+// keep their memset value 0, which makes the skip sticky. prev_inf == nullptr: no check (first slot of a batch,
+// bare oci_iterate / si_iterate calls).
+struct StopCheck {
+    const unsigned long long *prev_inf; // resid_inf[slot - 1]
+    const double *prev_l2;              // resid_l2[slot - 1]
+    const double *prev2_l2;             // resid_l2[slot - 2], nullptr if slot - 1 == 0 (Eq. 12 is tested from l >= 1)
+    double tol;
+    int rule;
+    int slot;
+    int *executed;                      // ctrl[0] <- slot + 1 by every iteration that runs
+};
+
 struct IterParams {
+    StopCheck stop;
     int J, N, G, n;
     int bc_left, bc_right;
     const double *Minv;
@@ -108,12 +127,13 @@ static inline ProblemView make_view(const oci_ctx *c)
 int launch_factor(oci_ctx *ctx);
 int launch_assemble_one(oci_ctx *ctx, int cell, double *A_dev_rowmajor);
 int launch_const_rhs(oci_ctx *ctx);
-int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2);
+int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
+StopCheck make_stop(const oci_ctx *ctx, int slot, bool check_prev);
 int launch_advance(oci_ctx *ctx);
 int launch_seed_iterate(oci_ctx *ctx);
 int launch_scalar_flux(oci_ctx *ctx, const double *psi, double *phi);
 int launch_si_setup(oci_ctx *ctx);
-int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2);
+int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 
 #ifdef __CUDACC__
 // ------------------------------------------------------------------------------------------------------------
@@ -126,6 +146,18 @@ __device__ __forceinline__ unsigned long long resid_bits(double d)
 {
     if (!(d == d)) d = __longlong_as_double(0x7ff0000000000000LL);
     return (unsigned long long)__double_as_longlong(d);
+}
+
+// Same arithmetic, operation by operation, as the host test in step_impl (api.cu).
+__device__ __forceinline__ bool stop_reached(const StopCheck &s)
+{
+    if (!s.prev_inf) return false;
+    if (s.rule == OCI_STOP_DPHI_INF) return __longlong_as_double((long long)*s.prev_inf) < s.tol;
+    if (!s.prev2_l2) return false;
+    const double e2 = *s.prev_l2, e2p = *s.prev2_l2;
+    if (e2 == 0.0 && e2p == 0.0) return true; // two skipped slots in a row
+    const double e = __dsqrt_rn(e2), ep = __dsqrt_rn(e2p);
+    return e < __dmul_rn(s.tol, __dsub_rn(1.0, __ddiv_rn(e, ep)));
 }
 
 __device__ __forceinline__ double warp_max(double v)

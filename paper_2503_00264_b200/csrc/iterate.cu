@@ -119,6 +119,8 @@ __device__ __forceinline__ double incident_term(const IterParams &P, const doubl
 template <bool WANT_L2>
 __global__ void __launch_bounds__(ITER_THREADS, 1) oci_iterate_stream_kernel(const IterParams P)
 {
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int n = P.n, N = P.N, G = P.G, J = P.J;
     const int cpb = P.cpb, S = P.S, nch = P.nch, stages = P.stages;
@@ -301,6 +303,8 @@ constexpr int WPC_MAX_STAGES = 16;                // WPC_WARPS x stages per warp
 template <int RPL, bool WANT_L2>
 __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const IterParams P)
 {
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
     constexpr int n = 32 * RPL;
     constexpr int CW = WPC_CHUNK / n;   // columns per chunk
     constexpr int NCH = n / CW;         // chunks per cell
@@ -465,6 +469,8 @@ __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const I
 template <bool WANT_L2>
 __global__ void __launch_bounds__(256) oci_iterate_plain_kernel(const IterParams P)
 {
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n = P.n, N = P.N, G = P.G, J = P.J;
     double *b = reinterpret_cast<double *>(smem_raw); // [n]
@@ -615,9 +621,10 @@ static StreamPlan make_plan(const oci_ctx *ctx)
     return pl;
 }
 
-int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2)
+int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev)
 {
     IterParams P;
+    P.stop = make_stop(ctx, hist_slot, check_prev);
     P.J = ctx->J; P.N = ctx->N; P.G = ctx->G; P.n = ctx->n;
     P.bc_left = ctx->bc_left; P.bc_right = ctx->bc_right;
     P.Minv = ctx->Minv; P.c = ctx->c;

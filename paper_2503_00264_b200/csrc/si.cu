@@ -88,10 +88,11 @@ __global__ void si_setup_kernel(ProblemView P, double *__restrict__ Linv, double
 }
 
 // a9: d_{j,g,m} (Eq. 43b-c, without the incident term) and base = Linv d.
-__global__ void si_source_kernel(ProblemView P, const double *__restrict__ q, const double *__restrict__ psi_prev,
-                                 const double *__restrict__ phi, const double *__restrict__ Linv,
-                                 double *__restrict__ base)
+__global__ void si_source_kernel(StopCheck stop, ProblemView P, const double *__restrict__ q,
+                                 const double *__restrict__ psi_prev, const double *__restrict__ phi,
+                                 const double *__restrict__ Linv, double *__restrict__ base)
 {
+    if (stop_reached(stop)) return;
     const size_t total = (size_t)P.J * P.G * P.N;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
         const size_t jg = e / P.N;
@@ -124,7 +125,7 @@ constexpr int LPC = 4;
 constexpr int TC = 32;
 constexpr int SW_STAGES = 4;
 
-__global__ void __launch_bounds__(32) si_sweep_kernel(int J, int N, int G, int bc_left, int bc_right,
+__global__ void __launch_bounds__(32) si_sweep_kernel(StopCheck stop, int J, int N, int G, int bc_left, int bc_right,
                                                       const double *__restrict__ mu, const double *__restrict__ C,
                                                       const double *__restrict__ base,
                                                       const double *__restrict__ psi_old,
@@ -132,6 +133,7 @@ __global__ void __launch_bounds__(32) si_sweep_kernel(int J, int N, int G, int b
                                                       const double *__restrict__ inc_right, double *__restrict__ in_out)
 {
     __shared__ __align__(16) double tile[SW_STAGES][TC][LPC][8]; // [C out0 (2)][C out1 (2)][base (4)]
+    if (stop_reached(stop)) return;
     const int lane = threadIdx.x;
     const int GN = G * N, n = 4 * GN;
     const int gm0 = blockIdx.x * LPC;
@@ -209,11 +211,13 @@ __global__ void __launch_bounds__(32) si_sweep_kernel(int J, int N, int G, int b
 constexpr int FIN_THREADS = 256;
 template <bool WANT_L2>
 __global__ void __launch_bounds__(FIN_THREADS)
-si_finish_kernel(int J, int N, int G, const double *__restrict__ w, const double *__restrict__ C,
+si_finish_kernel(StopCheck stop, int J, int N, int G, const double *__restrict__ w, const double *__restrict__ C,
                  const double *__restrict__ base, const double *__restrict__ in_, double *__restrict__ psi,
                  double *__restrict__ phi, unsigned long long *resid_inf, double *resid_l2)
 {
     __shared__ double ws[FIN_THREADS][4];
+    if (stop_reached(stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *stop.executed = stop.slot + 1;
     const int pairs_per_block = FIN_THREADS / N; // (j,g) pairs per block
     const size_t n_pairs = (size_t)J * G;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -274,16 +278,17 @@ int launch_si_setup(oci_ctx *ctx)
     return 1;
 }
 
-int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2)
+int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev)
 {
     ProblemView P = make_view(ctx);
+    const StopCheck stop = make_stop(ctx, hist_slot, check_prev);
     const int GN = ctx->G * ctx->N;
     const size_t total = (size_t)ctx->J * GN;
     double *psi = ctx->psi[ctx->cur];
-    si_source_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(P, ctx->q, ctx->psi_prev, ctx->phi,
+    si_source_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(stop, P, ctx->q, ctx->psi_prev, ctx->phi,
                                                                                    ctx->si_Linv, ctx->si_base);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
-    si_sweep_kernel<<<(GN + LPC - 1) / LPC, 32, 0, ctx->stream>>>(ctx->J, ctx->N, ctx->G, ctx->bc_left, ctx->bc_right,
+    si_sweep_kernel<<<(GN + LPC - 1) / LPC, 32, 0, ctx->stream>>>(stop, ctx->J, ctx->N, ctx->G, ctx->bc_left, ctx->bc_right,
                                                                   ctx->mu, ctx->si_T, ctx->si_base, psi, ctx->inc_left,
                                                                   ctx->inc_right, ctx->si_in);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
@@ -291,12 +296,12 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2)
     size_t blocks = ((size_t)ctx->J * ctx->G + pairs_per_block - 1) / pairs_per_block;
     if (blocks > (size_t)ctx->num_sms * 16) blocks = (size_t)ctx->num_sms * 16;
     if (want_l2)
-        si_finish_kernel<true><<<(int)blocks, FIN_THREADS, 0, ctx->stream>>>(ctx->J, ctx->N, ctx->G, ctx->w, ctx->si_T,
+        si_finish_kernel<true><<<(int)blocks, FIN_THREADS, 0, ctx->stream>>>(stop, ctx->J, ctx->N, ctx->G, ctx->w, ctx->si_T,
                                                                             ctx->si_base, ctx->si_in, psi, ctx->phi,
                                                                             ctx->resid_inf + hist_slot,
                                                                             ctx->resid_l2 + hist_slot);
     else
-        si_finish_kernel<false><<<(int)blocks, FIN_THREADS, 0, ctx->stream>>>(ctx->J, ctx->N, ctx->G, ctx->w, ctx->si_T,
+        si_finish_kernel<false><<<(int)blocks, FIN_THREADS, 0, ctx->stream>>>(stop, ctx->J, ctx->N, ctx->G, ctx->w, ctx->si_T,
                                                                              ctx->si_base, ctx->si_in, psi, ctx->phi,
                                                                              ctx->resid_inf + hist_slot,
                                                                              ctx->resid_l2 + hist_slot);

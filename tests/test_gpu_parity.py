@@ -185,3 +185,37 @@ def test_set_dt_refactors():
     s.iterate(2)
     o.oci_iterate(2)
     assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("scheme", ["oci", "si"])
+@pytest.mark.parametrize("k", [2, 5, 8])
+def test_device_side_stop_runs_the_natural_iteration_count(scheme, rule, k):
+    """DESIGN.md section 5 "device-side stop": with check_every = k the launches after the iteration at which the
+    rule first held skip themselves, so the iterations that ran, the converged iterate (whichever Jacobi buffer
+    it ended in) and the state handed to the next step equal the oracle's natural run."""
+    p = W.random_problem(33, 61, 4, 2, bc_left=1, bc_right=2, dt=0.05)
+    s, o = _solver(p), _oracle(p)
+    for step in range(3):
+        if scheme == "oci":
+            it_g, conv_g, _ = s.step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
+            it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule)
+        else:
+            it_g, conv_g, _ = s.si_step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
+            it_o, hist_o = o.si_step(tol=1e-9, max_iters=500, rule=rule)
+        assert it_g == conv_g == it_o, f"step {step}"
+        hist_g = s.residual_history(kind=rule)
+        assert len(hist_g) == it_o
+        np.testing.assert_allclose(hist_g, hist_o, rtol=1e-6, atol=1e-15)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_PHI
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+def test_max_iters_reached_without_convergence():
+    p = W.config2(dt=1.0, J=128)
+    s, o = _solver(p), _oracle(p)
+    it_g, conv_g, res = s.step(tol=1e-14, max_iters=13, check_every=4, advance=False)
+    assert (it_g, conv_g) == (13, 0)
+    o.factor(); o.const_rhs(); o.oci_iterate(13)
+    assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
