@@ -234,9 +234,9 @@ def run_ours(args):
     value = world * J * iters_total / (ms_total * 1e-3)
 
     # ---- SI comparator, same sequence (reported beside, not part of `value`) ----------------------------------
-    for i in range(Wm):
+    for i in range(0 if args.no_si else Wm):
         si.set_dt(SWEEP[i % len(SWEEP)]); si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
-    for i in range(Wm, Wm + K):
+    for i in range(Wm, Wm if args.no_si else Wm + K):
         dt = SWEEP[i % len(SWEEP)]
         si.set_dt(dt)
         torch.cuda.synchronize(); t = time.perf_counter()
@@ -244,7 +244,7 @@ def run_ours(args):
         el = (time.perf_counter() - t) * 1e3
         per_dt[dt].setdefault("si_iters", []).append(it)
         per_dt[dt].setdefault("si_ms", []).append(el)
-    diff = float((oci.scalar_flux() - si.scalar_flux()).abs().max().item())
+    diff = None if args.no_si else float((oci.scalar_flux() - si.scalar_flux()).abs().max().item())
 
     # ---- end-to-end leg: host buffers through oci_step_host, copies inside the timed region ------------------
     e2e = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}")
@@ -331,6 +331,7 @@ def main():
     ap.add_argument("--cpu-cells", type=int, default=32768, help="cells of the cpu_baseline sample")
     ap.add_argument("--ref-cells", type=int, default=8192, help="cells per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-si", action="store_true", help="skip the SI comparator leg (profiling runs)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
