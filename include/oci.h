@@ -86,8 +86,8 @@ int oci_last_cuda_error(const oci_ctx *ctx);
 /* Tuning knobs (all optional). Known keys: "iterate_kernel" (0 = plain one-CTA-per-cell, 1 = pipelined
  * bulk-copy streaming kernel [default]), "iterate_stages", "iterate_ctas_per_sm", "factor_kernel"
  * (0 = shared-memory elimination, 1 = auto), "use_graph", "refactor_every_step" (1 = oci_step / si_step redo
- * a1+a2 at the start of every step as Alg. 2 prints it; 0 [default] = only when dt changed). Returns -2 for an
- * unknown key. */
+ * a1+a2 at the start of every step as Alg. 2 prints it; 0 [default] = only when dt changed), "si_lanes" (ordinates x
+ * groups swept by one CTA of the SI sweep kernel: 4, 8 [default] or 16). Returns -2 for an unknown key. */
 int oci_set_option(oci_ctx *ctx, const char *key, int64_t value);
 
 int oci_set_dt(oci_ctx *ctx, double dt);                               /* invalidates the factors      */

@@ -86,6 +86,9 @@ size_t carve(oci_ctx *c, unsigned char *base, int J, int N, int G, int num_sms, 
     t->si_T = cv.take<double>((size_t)J * GN * 8);
     t->si_base = cv.take<double>((size_t)J * GN * 4);
     t->si_in = cv.take<double>((size_t)J * GN * 2);
+    const size_t GNpad = (GN + 15) / 16 * 16; // room for any "si_lanes" grouping (4, 8, 16)
+    t->si_T2sw = cv.take<double>((size_t)J * GNpad * 4);
+    t->si_bsw = cv.take<double>((size_t)J * GNpad * 2);
     t->resid_inf = cv.take<unsigned long long>(OCI_RESID_CAP);
     t->resid_l2 = cv.take<double>(OCI_RESID_CAP);
     t->ctrl = cv.take<int>(4);
@@ -363,6 +366,7 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     else if (!strcmp(key, "factor_kernel")) ctx->opt_factor_kernel = (int)value;
     else if (!strcmp(key, "use_graph")) ctx->opt_use_graph = (int)value;
     else if (!strcmp(key, "refactor_every_step")) ctx->opt_refactor_every_step = (int)value;
+    else if (!strcmp(key, "si_lanes")) { ctx->opt_si_lanes = (int)value; ctx->si_valid = false; }
     else return -2;
     return 0;
 }

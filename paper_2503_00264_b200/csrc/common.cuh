@@ -47,6 +47,8 @@ struct oci_ctx {
     double *si_T;       // [J][G*N][4][2] C = |mu| Linv[:, incident rows]; its outgoing rows are the sweep's 2x2 map
     double *si_base;    // [J][G*N][4]    Linv * d (no incident term)
     double *si_in;      // [J][G*N][2]    incident edge flux of cell j found by the sweep
+    double *si_T2sw;    // [ceil(GN/lpc)][J][lpc][2][2]  incident -> outgoing 2x2 map, sweep order (si.cu sweep_index)
+    double *si_bsw;     // [ceil(GN/lpc)][J][lpc][2]     outgoing entries of si_base, sweep order
     // residual history (device) + pinned host mirror
     unsigned long long *resid_inf; // [OCI_RESID_CAP] bit pattern of a non-negative double
     double *resid_l2;              // [OCI_RESID_CAP] sum of squares
@@ -60,7 +62,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph, opt_refactor_every_step;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph, opt_refactor_every_step, opt_si_lanes;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];
@@ -177,6 +179,59 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// ---- mbarrier / bulk-copy PTX wrappers ---------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// Bounded wait: a protocol bug traps (-> CUDA error) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    unsigned long long t0 = 0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if ((++spins & 0x3ff) == 0) {
+            unsigned long long t1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+            if (t1 - t0 > 4000000000ULL) __trap(); // 4 s
+        }
+    }
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
 // Eq. 8b, PAPER.md:132 -- entry (p, pp) of the 4x4 within-cell block L_{c,j,g,m}. Every operation is an
 // explicitly rounded intrinsic so that the assembled matrix is bit-identical to a plain (uncontracted)
 // evaluation of the same formula.

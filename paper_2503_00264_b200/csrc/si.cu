@@ -54,9 +54,20 @@ __device__ __forceinline__ void inv4(double (&a)[4][4], double (&b)[4][4])
     }
 }
 
-// Once per (problem, dt): Linv[j][g][m][4][4] = L_{c,j,g,m}^{-1} (Eq. 8b / 42) and
-// C[j][g][m][p][lev] = |mu_m| Linv[p][row that receives the incident flux of level lev].
-__global__ void si_setup_kernel(ProblemView P, double *__restrict__ Linv, double *__restrict__ C)
+// Sweep-order record index of (cell j, ordinate gm): chains are grouped `lpc` to a CTA; within a CTA's slab the
+// records of one sweep step jj (cell jj for mu > 0, cell J-1-jj for mu < 0) of its lpc chains are contiguous, so a
+// tile of consecutive sweep steps is ONE contiguous block that a single bulk copy brings into shared memory.
+__device__ __forceinline__ size_t sweep_index(int J, int lpc, size_t j, int gm, bool fwd)
+{
+    const size_t jj = fwd ? j : (size_t)(J - 1) - j;
+    return ((size_t)(gm / lpc) * J + jj) * lpc + (gm % lpc);
+}
+
+// Once per (problem, dt): Linv[j][g][m][4][4] = L_{c,j,g,m}^{-1} (Eq. 8b / 42),
+// C[j][g][m][p][lev] = |mu_m| Linv[p][row that receives the incident flux of level lev], and the 2x2 part of C
+// that maps incident -> outgoing edge flux, T2sw[sweep_index][2][2], in sweep order for si_sweep_kernel.
+__global__ void si_setup_kernel(ProblemView P, int lpc, double *__restrict__ Linv, double *__restrict__ C,
+                                double *__restrict__ T2sw)
 {
     const size_t total = (size_t)P.J * P.G * P.N;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
@@ -84,13 +95,20 @@ __global__ void si_setup_kernel(ProblemView P, double *__restrict__ Linv, double
             Co[p * 2 + 0] = am * (mu > 0.0 ? b[p][0] : b[p][1]);
             Co[p * 2 + 1] = am * (mu > 0.0 ? b[p][2] : b[p][3]);
         }
+        // outgoing unknowns: (k,R),(k+1/2,R) = rows 1,3 for mu > 0; (k,L),(k+1/2,L) = rows 0,2 for mu < 0 (Eq. 5a-b)
+        const bool fwd = mu > 0.0;
+        const int o0 = fwd ? 1 : 0;
+        double *To = T2sw + sweep_index(P.J, lpc, j, g * P.N + m, fwd) * 4;
+        reinterpret_cast<double2 *>(To)[0] = make_double2(Co[o0 * 2], Co[o0 * 2 + 1]);
+        reinterpret_cast<double2 *>(To)[1] = make_double2(Co[(o0 + 2) * 2], Co[(o0 + 2) * 2 + 1]);
     }
 }
 
 // a9: d_{j,g,m} (Eq. 43b-c, without the incident term) and base = Linv d.
-__global__ void si_source_kernel(StopCheck stop, ProblemView P, const double *__restrict__ q,
+__global__ void si_source_kernel(StopCheck stop, ProblemView P, int lpc, const double *__restrict__ q,
                                  const double *__restrict__ psi_prev, const double *__restrict__ phi,
-                                 const double *__restrict__ Linv, double *__restrict__ base)
+                                 const double *__restrict__ Linv, double *__restrict__ base,
+                                 double *__restrict__ bsw)
 {
     if (stop_reached(stop)) return;
     const size_t total = (size_t)P.J * P.G * P.N;
@@ -112,57 +130,76 @@ __global__ void si_source_kernel(StopCheck stop, ProblemView P, const double *__
         d[0] = fma(half_gam, psi_prev[e * 2 + 0], d[0]);
         d[1] = fma(half_gam, psi_prev[e * 2 + 1], d[1]);
         const double *L = Linv + e * 16;
+        double bs[4];
 #pragma unroll
-        for (int p = 0; p < 4; ++p)
-            base[e * 4 + p] = fma(L[p * 4 + 3], d[3], fma(L[p * 4 + 2], d[2], fma(L[p * 4 + 1], d[1], L[p * 4 + 0] * d[0])));
+        for (int p = 0; p < 4; ++p) {
+            bs[p] = fma(L[p * 4 + 3], d[3], fma(L[p * 4 + 2], d[2], fma(L[p * 4 + 1], d[1], L[p * 4 + 0] * d[0])));
+            base[e * 4 + p] = bs[p];
+        }
+        // the two outgoing entries of base, in sweep order (the constant term of the sweep's 2x2 affine map)
+        const int m = (int)(e % P.N);
+        const bool fwd = P.mu[m] > 0.0;
+        *reinterpret_cast<double2 *>(bsw + sweep_index(P.J, lpc, j, g * P.N + m, fwd) * 2) =
+            fwd ? make_double2(bs[1], bs[3]) : make_double2(bs[0], bs[2]);
     }
 }
 
-// a10: the sweep. One warp per CTA sweeps LPC ordinates (g,m): all 32 lanes stage the per-cell 2x2 maps and
-// base values of the next cells into a shared-memory ring with cp.async (the loads do not depend on the
-// chain), the first LPC lanes run the serial chain out of shared memory.
-constexpr int LPC = 4;
-constexpr int TC = 32;
+// a10: the sweep. One CTA per group of LPC chains (ordinates (g,m)), warp-specialised:
+//   warp 1, one thread : issues one bulk async copy per tile (TC sweep steps x LPC chains) of the 2x2 maps and one of
+//                        the constant terms into a ring of SW_STAGES shared-memory stages (mbarrier handshake);
+//   warp 0, lane = chain: runs the serial chain  in_{jj+1} = b_jj + T_jj in_jj  out of shared memory -- per cell three
+//                        conflict-free 16-byte loads, four DFMAs (two dependent), one 16-byte store of the incident
+//                        flux that si_finish needs. Nothing else is on the chain warp's instruction stream.
+// The chain is the latency floor of a sweep "serial in space": J x 2 dependent DFMAs.
+constexpr int TC = 64;         // sweep steps per tile
 constexpr int SW_STAGES = 4;
+constexpr int SW_THREADS = 64;
 
-__global__ void __launch_bounds__(32) si_sweep_kernel(StopCheck stop, int J, int N, int G, int bc_left, int bc_right,
-                                                      const double *__restrict__ mu, const double *__restrict__ C,
-                                                      const double *__restrict__ base,
-                                                      const double *__restrict__ psi_old,
-                                                      const double *__restrict__ inc_left,
-                                                      const double *__restrict__ inc_right, double *__restrict__ in_out)
+template <int LPC>
+__global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, int J, int N, int G, int bc_left,
+                                                              int bc_right, const double *__restrict__ mu,
+                                                              const double *__restrict__ T2sw,
+                                                              const double *__restrict__ bsw,
+                                                              const double *__restrict__ psi_old,
+                                                              const double *__restrict__ inc_left,
+                                                              const double *__restrict__ inc_right,
+                                                              double *__restrict__ in_out)
 {
-    __shared__ __align__(16) double tile[SW_STAGES][TC][LPC][8]; // [C out0 (2)][C out1 (2)][base (4)]
+    extern __shared__ __align__(128) unsigned char sw_smem[];
+    typedef double (*TsT)[TC][LPC][4];
+    typedef double (*BsT)[TC][LPC][2];
+    TsT Ts = reinterpret_cast<TsT>(sw_smem);                                              // [SW_STAGES][TC][LPC][4]
+    BsT Bs = reinterpret_cast<BsT>(sw_smem + sizeof(double) * SW_STAGES * TC * LPC * 4); // [SW_STAGES][TC][LPC][2]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sw_smem + sizeof(double) * SW_STAGES * TC * LPC * 6);
+    uint64_t *empty = full + SW_STAGES;
     if (stop_reached(stop)) return;
-    const int lane = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int GN = G * N, n = 4 * GN;
     const int gm0 = blockIdx.x * LPC;
     const int n_tiles = (J + TC - 1) / TC;
+    if (tid == 0) {
+        for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        fence_mbar_init();
+    }
+    __syncthreads();
 
-    auto stage_tile = [&](int t) {
-        if (t < n_tiles) {
-            double(*dst)[LPC][8] = tile[t % SW_STAGES];
-            for (int idx = lane; idx < TC * LPC * 4; idx += 32) {
-                const int part = idx & 3, l = (idx >> 2) % LPC, u = idx / (4 * LPC);
-                const int gm = gm0 + l, jj = t * TC + u;
-                if (gm < GN && jj < J) {
-                    const bool fwd = mu[gm % N] > 0.0;
-                    const size_t j = fwd ? jj : J - 1 - jj;
-                    const size_t cell_gm = j * GN + gm;
-                    const int o0 = fwd ? 1 : 0; // outgoing unknowns: (k,R),(k+1/2,R) for mu>0; (k,L),(k+1/2,L) for mu<0
-                    const double *src = part == 0   ? C + cell_gm * 8 + o0 * 2
-                                        : part == 1 ? C + cell_gm * 8 + (o0 + 2) * 2
-                                        : part == 2 ? base + cell_gm * 4
-                                                    : base + cell_gm * 4 + 2;
-                    const uint32_t d = smem_u32(&dst[u][l][part * 2]);
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
-                }
+    if (warp == 1) {
+        if (lane == 0) {
+            const double *Tsrc = T2sw + (size_t)blockIdx.x * J * LPC * 4;
+            const double *Bsrc = bsw + (size_t)blockIdx.x * J * LPC * 2;
+            for (int t = 0; t < n_tiles; ++t) {
+                const int st = t % SW_STAGES;
+                mbar_wait(&empty[st], ((t / SW_STAGES) & 1) ^ 1);
+                const int cells = min(TC, J - t * TC);
+                const uint32_t bt = (uint32_t)(cells * LPC * 4 * sizeof(double));
+                const uint32_t bb = (uint32_t)(cells * LPC * 2 * sizeof(double));
+                mbar_arrive_expect_tx(&full[st], bt + bb);
+                bulk_g2s(&Ts[st][0][0][0], Tsrc + (size_t)t * TC * LPC * 4, bt, &full[st]);
+                bulk_g2s(&Bs[st][0][0][0], Bsrc + (size_t)t * TC * LPC * 2, bb, &full[st]);
             }
         }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    };
-
-    for (int t = 0; t < SW_STAGES - 1; ++t) stage_tile(t);
+        return;
+    }
 
     const int gm = gm0 + lane;
     const bool active = lane < LPC && gm < GN;
@@ -182,28 +219,45 @@ __global__ void __launch_bounds__(32) si_sweep_kernel(StopCheck stop, int J, int
             in1 = ip[1];
         }
     }
+    // in_out[j][gm][2]: element stride between consecutive sweep steps of this chain
+    const long long ostep = fwd ? (long long)GN * 2 : -(long long)GN * 2;
+    double *op = in_out + ((fwd ? (size_t)0 : (size_t)(J - 1)) * GN + (active ? gm : 0)) * 2;
+    const int l = active ? lane : 0;
 
     for (int t = 0; t < n_tiles; ++t) {
-        stage_tile(t + SW_STAGES - 1);
-        asm volatile("cp.async.wait_group %0;" ::"n"(SW_STAGES - 1) : "memory");
-        __syncwarp();
+        const int st = t % SW_STAGES;
+        mbar_wait(&full[st], (t / SW_STAGES) & 1);
+        const int cells = min(TC, J - t * TC);
         if (active) {
-            const double(*src)[LPC][8] = tile[t % SW_STAGES];
-            const int cells = min(TC, J - t * TC);
-#pragma unroll 8
-            for (int u = 0; u < cells; ++u) {
-                const double *s = src[u][lane];
-                const int jj = t * TC + u;
-                const size_t j = fwd ? jj : J - 1 - jj;
-                *reinterpret_cast<double2 *>(in_out + (j * GN + gm) * 2) = make_double2(in0, in1);
-                const int ob = fwd ? 1 : 0;
-                const double o0 = fma(s[0], in0, fma(s[1], in1, s[4 + ob]));
-                const double o1 = fma(s[2], in0, fma(s[3], in1, s[4 + ob + 2]));
-                in0 = o0;
-                in1 = o1;
+            if (cells == TC) {
+#pragma unroll 16
+                for (int u = 0; u < TC; ++u) {
+                    const double2 t0 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][0]);
+                    const double2 t1 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][2]);
+                    const double2 bb = *reinterpret_cast<const double2 *>(&Bs[st][u][l][0]);
+                    *reinterpret_cast<double2 *>(op) = make_double2(in0, in1);
+                    op += ostep;
+                    const double o0 = fma(t0.x, in0, fma(t0.y, in1, bb.x));
+                    const double o1 = fma(t1.x, in0, fma(t1.y, in1, bb.y));
+                    in0 = o0;
+                    in1 = o1;
+                }
+            } else {
+                for (int u = 0; u < cells; ++u) {
+                    const double2 t0 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][0]);
+                    const double2 t1 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][2]);
+                    const double2 bb = *reinterpret_cast<const double2 *>(&Bs[st][u][l][0]);
+                    *reinterpret_cast<double2 *>(op) = make_double2(in0, in1);
+                    op += ostep;
+                    const double o0 = fma(t0.x, in0, fma(t0.y, in1, bb.x));
+                    const double o1 = fma(t1.x, in0, fma(t1.y, in1, bb.y));
+                    in0 = o0;
+                    in1 = o1;
+                }
             }
         }
         __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);
     }
 }
 
@@ -269,11 +323,19 @@ inline int grid_for(size_t total, int threads, int num_sms)
 
 } // namespace
 
+// chains (ordinates x groups) per sweep CTA: 4, 8 or 16 ("si_lanes" option; default 8)
+static int si_lanes(const oci_ctx *ctx)
+{
+    const int v = ctx->opt_si_lanes;
+    return (v == 4 || v == 16) ? v : 8;
+}
+
 int launch_si_setup(oci_ctx *ctx)
 {
     ProblemView P = make_view(ctx);
     const size_t total = (size_t)ctx->J * ctx->G * ctx->N;
-    si_setup_kernel<<<grid_for(total, 128, ctx->num_sms), 128, 0, ctx->stream>>>(P, ctx->si_Linv, ctx->si_T);
+    si_setup_kernel<<<grid_for(total, 128, ctx->num_sms), 128, 0, ctx->stream>>>(P, si_lanes(ctx), ctx->si_Linv, ctx->si_T,
+                                                                                 ctx->si_T2sw);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
     return 1;
 }
@@ -285,12 +347,29 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_pr
     const int GN = ctx->G * ctx->N;
     const size_t total = (size_t)ctx->J * GN;
     double *psi = ctx->psi[ctx->cur];
-    si_source_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(stop, P, ctx->q, ctx->psi_prev, ctx->phi,
-                                                                                   ctx->si_Linv, ctx->si_base);
+    const int lpc = si_lanes(ctx);
+    si_source_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(stop, P, lpc, ctx->q, ctx->psi_prev,
+                                                                                   ctx->phi, ctx->si_Linv, ctx->si_base,
+                                                                                   ctx->si_bsw);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
-    si_sweep_kernel<<<(GN + LPC - 1) / LPC, 32, 0, ctx->stream>>>(stop, ctx->J, ctx->N, ctx->G, ctx->bc_left, ctx->bc_right,
-                                                                  ctx->mu, ctx->si_T, ctx->si_base, psi, ctx->inc_left,
-                                                                  ctx->inc_right, ctx->si_in);
+    const int sweep_grid = (GN + lpc - 1) / lpc;
+#define OCI_SWEEP(LPC_)                                                                                            \
+    do {                                                                                                           \
+        const size_t smem = sizeof(double) * SW_STAGES * TC * LPC_ * 6 + 2 * SW_STAGES * sizeof(uint64_t);         \
+        static bool attr_set = false;                                                                              \
+        if (!attr_set) {                                                                                           \
+            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(si_sweep_kernel<LPC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                                   (int)smem));                                                    \
+            attr_set = true;                                                                                       \
+        }                                                                                                          \
+        si_sweep_kernel<LPC_><<<sweep_grid, SW_THREADS, smem, ctx->stream>>>(                                       \
+            stop, ctx->J, ctx->N, ctx->G, ctx->bc_left, ctx->bc_right, ctx->mu, ctx->si_T2sw, ctx->si_bsw, psi,      \
+            ctx->inc_left, ctx->inc_right, ctx->si_in);                                                            \
+    } while (0)
+    if (lpc == 4) OCI_SWEEP(4);
+    else if (lpc == 8) OCI_SWEEP(8);
+    else OCI_SWEEP(16);
+#undef OCI_SWEEP
     OCI_CUDA_TRY(ctx, cudaGetLastError());
     const int pairs_per_block = FIN_THREADS / ctx->N;
     size_t blocks = ((size_t)ctx->J * ctx->G + pairs_per_block - 1) / pairs_per_block;
