@@ -151,6 +151,114 @@ namespace cg = cooperative_groups;
 constexpr int FR_THREADS = 256;
 constexpr int FR_NB = 8;
 
+// Branch-free reciprocal: hardware seed (MUFU.RCP64H, ~2^-20) + one cubic and one quadratic Newton step, accurate to
+// about an ulp for normal x. No special cases: zero / non-finite pivots are flagged separately as singular.
+__device__ __forceinline__ double rcp_nr(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    e = fma(e, e, e);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+
+// Phase P of the blocked Gauss-Jordan (both register-tiled kernels): one warp eliminates its n x 8 panel `a`
+// (lane l holds the rows {64 s + 2 l, 64 s + 2 l + 1}, s < TR / 2, register row rr = 2 s + e) with warp-level
+// operations only. usedmask: bit rr set = that row of this lane was a pivot row of an earlier step. bc: 20 doubles of
+// shared memory private to the warp. Returns the pivot rows in Rl and whether a zero / non-finite pivot was met.
+template <int TR>
+__device__ __forceinline__ bool panel_eliminate(double (&a)[TR][8], unsigned usedmask, double *bc, int lane,
+                                                int (&Rl)[FR_NB])
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    // Everything that does not depend on WHICH row wins (1/candidate, the candidate row scaled by it)
+    // is computed by every lane for its own candidate in the shadow of the arg-max reduction; the
+    // winner then only has to publish 64 bytes.
+    bool bad = false;
+    unsigned um = usedmask;
+#pragma unroll
+    for (int b = 0; b < FR_NB; ++b) {
+        // local candidate: first row of maximal |entry| among this lane's unused rows
+        unsigned long long bk = 0ull;
+        int brr = -1;
+#pragma unroll
+        for (int rr = 0; rr < TR; ++rr) {
+            const unsigned long long key = (unsigned long long)__double_as_longlong(fabs(a[rr][b]));
+            if (!((um >> rr) & 1u) && (brr < 0 || key > bk)) { bk = key; brr = rr; }
+        }
+        const bool valid = brr >= 0;
+        const unsigned khi = valid ? (unsigned)(bk >> 32) : 0u;
+        const unsigned mhi = __reduce_max_sync(FULL, khi);
+        // (independent of the reduction) the candidate row, scaled by 1/candidate; column b holds 1/candidate
+        double scl[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            double v = a[0][c];
+#pragma unroll
+            for (int rr = 1; rr < TR; ++rr) v = (brr == rr) ? a[rr][c] : v;
+            scl[c] = v;
+        }
+        const double linv = rcp_nr(scl[b]);
+#pragma unroll
+        for (int c = 0; c < 8; ++c) scl[c] = (c == b) ? linv : scl[c] * linv;
+        const unsigned bit0 = __ballot_sync(FULL, brr & 1), bit1 = __ballot_sync(FULL, brr & 2),
+                       bit2 = __ballot_sync(FULL, brr & 4);
+        // winner: the only lane whose high key word equals the maximum (common case), else exact
+        bool cand = valid && khi == mhi;
+        const unsigned ball = __ballot_sync(FULL, cand);
+        int src;
+        if (__popc(ball) == 1) {
+            src = __ffs(ball) - 1;
+        } else { // ties in the high word (or no valid row): compare the low words, then the lowest row
+            const unsigned klo = (unsigned)bk;
+            const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
+            cand = cand && klo == mlo;
+            const int row = cand ? 64 * (brr >> 1) + 2 * lane + (brr & 1) : INT_MAX;
+            const int rmin = __reduce_min_sync(FULL, row);
+            src = rmin == INT_MAX ? 0 : (rmin & 63) >> 1;
+        }
+        if (mhi == 0u || mhi >= 0x7ff00000u) bad = true; // zero / denormal, inf or NaN pivot
+        const int rr_r = (int)(((bit0 >> src) & 1u) | (((bit1 >> src) & 1u) << 1) | (((bit2 >> src) & 1u) << 2)) &
+                         (TR - 1); // warp-uniform
+        Rl[b] = 64 * (rr_r >> 1) + 2 * src + (rr_r & 1);
+        const bool mine = lane == src;
+        // pivot row (already scaled) through a per-warp shared-memory slot (two slots alternate)
+        double *slot = bc + (b & 1) * 10;
+        if (mine) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                reinterpret_cast<double2 *>(slot)[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
+        }
+        __syncwarp();
+        double sp[8];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const double2 t = reinterpret_cast<const double2 *>(slot)[c];
+            sp[2 * c] = t.x;
+            sp[2 * c + 1] = t.y;
+        }
+#pragma unroll
+        for (int rr = 0; rr < TR; ++rr) {
+            const bool is_p = mine && rr == rr_r;
+            const double f = is_p ? 0.0 : a[rr][b];
+            const double g = is_p ? linv : 1.0; // the pivot row becomes itself / pivot
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                if (c == b) {
+                    const double t = -f * sp[b];
+                    a[rr][c] = is_p ? linv : t;
+                } else {
+                    a[rr][c] = fma(-f, sp[c], a[rr][c] * g);
+                }
+            }
+        }
+        if (mine) um |= 1u << rr_r;
+    }
+    return bad;
+}
+
 template <int NQ> struct FrShared {
     double Z[2][FR_NB][64 * NQ];          // [buf][b][row]
     double Rrow[2][FR_NB][64];            // [buf][b][local column]
@@ -236,71 +344,7 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
             if (owner) {
                 // ================= phase P: eliminate the n x 8 panel inside this warp =====================
                 int Rl[FR_NB];
-                bool bad = false;
-                unsigned um = usedmask;
-                double *bc = &sh.bcast[w][0][0];
-#pragma unroll
-                for (int b = 0; b < FR_NB; ++b) {
-                    // local candidate: first row of maximal |entry| among this lane's unused rows
-                    unsigned long long bk = 0ull;
-                    int brow = INT_MAX;
-                    double bval = 1.0;
-#pragma unroll
-                    for (int rr = 0; rr < TR; ++rr) {
-                        const unsigned long long key = (unsigned long long)__double_as_longlong(fabs(a[rr][b]));
-                        if (!((um >> rr) & 1u) && (brow == INT_MAX || key > bk)) {
-                            bk = key;
-                            brow = 64 * (rr >> 1) + 2 * lane + (rr & 1);
-                            bval = a[rr][b];
-                        }
-                    }
-                    const double linv = 1.0 / bval; // of the lane's own candidate: overlaps the arg-max below
-                    const unsigned khi = (unsigned)(bk >> 32), klo = (unsigned)bk;
-                    const unsigned mhi = __reduce_max_sync(FULL, brow == INT_MAX ? 0u : khi);
-                    const bool c1 = brow != INT_MAX && khi == mhi;
-                    const unsigned mlo = __reduce_max_sync(FULL, c1 ? klo : 0u);
-                    const bool c2 = c1 && klo == mlo;
-                    const int r = __reduce_min_sync(FULL, c2 ? brow : INT_MAX);
-                    const unsigned long long mk = ((unsigned long long)mhi << 32) | mlo;
-                    if (mk == 0ull || mk >= 0x7ff0000000000000ull) bad = true; // zero, inf or NaN pivot
-                    Rl[b] = r;
-                    const int lane_r = (r & 63) >> 1, rr_r = 2 * (r >> 6) + (r & 1); // warp-uniform
-                    const bool mine = lane == lane_r;
-                    // pivot row and 1/pivot through a per-warp shared-memory slot (two slots alternate)
-                    double *slot = bc + (b & 1) * 10;
-#pragma unroll
-                    for (int rr = 0; rr < TR; ++rr)
-                        if (rr == rr_r && mine) {
-#pragma unroll
-                            for (int c = 0; c < 4; ++c)
-                                reinterpret_cast<double2 *>(slot)[c] = make_double2(a[rr][2 * c], a[rr][2 * c + 1]);
-                            slot[8] = linv;
-                        }
-                    __syncwarp();
-                    double sp[8];
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        const double2 t = reinterpret_cast<const double2 *>(slot)[c];
-                        sp[2 * c] = t.x;
-                        sp[2 * c + 1] = t.y;
-                    }
-                    const double inv = slot[8];
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) sp[c] = (c == b) ? inv : sp[c] * inv;
-#pragma unroll
-                    for (int rr = 0; rr < TR; ++rr) {
-                        const double f = a[rr][b];
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) a[rr][c] = (c == b) ? -f * inv : fma(-f, sp[c], a[rr][c]);
-                    }
-#pragma unroll
-                    for (int rr = 0; rr < TR; ++rr)
-                        if (rr == rr_r && mine) {
-#pragma unroll
-                            for (int c = 0; c < 8; ++c) a[rr][c] = sp[c];
-                        }
-                    if (mine) um |= 1u << rr_r;
-                }
+                const bool bad = panel_eliminate<TR>(a, usedmask, &sh.bcast[w][0][0], lane, Rl);
                 // ---- publish Z = T[:, R] - I[:, R], R and the singular flag to every CTA of the cluster
 #pragma unroll
                 for (int t = 0; t < NQ; ++t) {
@@ -342,7 +386,7 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
                 }
                 if (w == 0 && lane == b) { sh.rho[FR_NB * pnl + b] = r; sh.rhoinv[r] = FR_NB * pnl + b; }
             }
-            __syncthreads(); // B2: Rrow of this CTA complete
+            __syncwarp(); // Rrow[.][.][8 w ..] is written and read by warp w alone
 
             if (!owner) {
                 // ================= phase U: rank-8 update of this thread's TR x 8 tile =======================
@@ -365,6 +409,7 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
             }
         }
 
+        __syncthreads(); // rho / rhoinv (written by warp 0 after each panel's B1) visible to every warp of the CTA
         double *out = Minv + (size_t)cell * n * n;
         if (singular) {
             if (q == 0 && threadIdx.x == 0) atomicMin(info, cell + 1);
@@ -382,6 +427,171 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
             double *col = out + (size_t)sh.rho[64 * q + 8 * w + c] * n;
 #pragma unroll
             for (int rr = 0; rr < TR; ++rr) col[ro[rr]] = a[rr][c];
+        }
+    }
+}
+
+// ============================================================================================================
+// n = 64: two warps per cell, the production a1 + a2 kernel of the headline configuration.
+// ============================================================================================================
+// Same blocked Gauss-Jordan as factor_reg_kernel, re-tiled so that MORE CELLS are in flight per SM: the owner's
+// panel phase is a serial, latency-bound instruction stream, so the throughput of the kernel is (cells in flight
+// per SM) / (length of that stream). Lane l of warp w holds the rows {2 l, 2 l + 1} of the columns
+// [32 w, 32 w + 32): 64 doubles per lane, 64 threads and ~17 KB of shared memory per cell, five cells per SM
+// (factor_reg_kernel<1>: three). Panel p (8 columns) belongs to warp p / 4, sub-tile p % 4 of its registers; the
+// owner copies that sub-tile out, eliminates it (panel_eliminate), publishes Z and R, and both warps apply the
+// rank-8 update to all their 32 columns (the owner then puts the eliminated sub-tile back over the result).
+constexpr int W2_THREADS = 64;
+
+struct W2Shared {
+    double S[2][32][64];           // [warp][local column][row]: shadow copy of the warp's tile, refreshed every panel
+    double Z[2][FR_NB][64];        // [buf][b][row]
+    double bcast[2][20];
+    int R[2][FR_NB];
+    int sing[2];
+    int rho[64], rhoinv[64];
+};
+
+__global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restrict__ Minv, int *info)
+{
+    constexpr int n = 64, NPANEL = n / FR_NB;
+    extern __shared__ __align__(16) unsigned char w2_smem[];
+    W2Shared &sh = *reinterpret_cast<W2Shared *>(w2_smem);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int N = P.N, G = P.G;
+    unsigned gp = 0;
+
+    for (int cell = blockIdx.x; cell < P.J; cell += gridDim.x) {
+        // ---- a1: assemble rows {2 lane, 2 lane + 1} x columns [32 w, 32 w + 32), bit-identical to a_entry().
+        // Register layout a[local column][row parity]: the two rows of a column are adjacent (16-byte stores).
+        double a[32][2];
+        {
+            const double dx = P.dx[cell];
+            const int p0 = (lane & 1) * 2;
+            const int bm = lane >> 1, m = bm % N, g = bm / N;
+            const double sig = P.sigma_t[(size_t)cell * G + g], mu = P.mu[m];
+            const double av = __dmul_rn(__dadd_rn(fabs(mu), __dmul_rn(dx, sig)), 0.5);
+            const double gam = __ddiv_rn(dx, __dmul_rn(P.v[g], P.dt));
+            const double h = __dmul_rn(mu, 0.5), hg = __dmul_rn(gam, 0.5), ga = __dadd_rn(gam, av);
+#pragma unroll
+            for (int cb = 0; cb < 8; ++cb) { // column block (g', m') = 8 w + cb
+                const int bmc = 8 * w + cb;
+                const double K = P.transfer[((size_t)cell * G + g) * G + bmc / N];
+                const double Kw = __dmul_rn(__dmul_rn(__dmul_rn(dx, K), 0.25), P.w[bmc % N]);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int p = p0 + e;
+#pragma unroll
+                    for (int pp = 0; pp < 4; ++pp) {
+                        double val = 0.0;
+                        if (bm == bmc) { // Eq. 8b
+                            const int d = pp - p;
+                            if (d == 0) val = p < 2 ? av : ga;
+                            else if (p == 0 && pp == 1) val = h;
+                            else if (p == 1 && pp == 0) val = -h;
+                            else if (p == 2 && pp == 3) val = h;
+                            else if (p == 3 && pp == 2) val = -h;
+                            else if (d == 2) val = hg;
+                            else if (d == -2) val = -gam;
+                        }
+                        if (p == pp) val = __dsub_rn(val, Kw);
+                        a[4 * cb + pp][e] = val;
+                    }
+                }
+            }
+        }
+        unsigned usedmask = 0;
+        bool singular = false;
+        double2 *Sw = reinterpret_cast<double2 *>(&sh.S[w][0][0]); // [local column][32 lanes] of double2
+
+        for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
+            const int buf = gp & 1;
+            const bool owner = (pnl >> 2) == w;
+            const int st = pnl & 3;
+            if (owner) {
+                double t[2][8];
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (k == st) {
+#pragma unroll
+                        for (int e = 0; e < 2; ++e)
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) t[e][c] = a[8 * k + c][e];
+                    }
+                int Rl[FR_NB];
+                const bool bad = panel_eliminate<2>(t, usedmask, &sh.bcast[w][0], lane, Rl);
+#pragma unroll
+                for (int b = 0; b < FR_NB; ++b) {
+                    double2 z;
+                    z.x = t[0][b] - (Rl[b] == 2 * lane ? 1.0 : 0.0);
+                    z.y = t[1][b] - (Rl[b] == 2 * lane + 1 ? 1.0 : 0.0);
+                    *reinterpret_cast<double2 *>(&sh.Z[buf][b][2 * lane]) = z;
+                    if (lane == b) sh.R[buf][b] = Rl[b];
+                }
+                if (lane == 0) sh.sing[buf] = bad ? 1 : 0;
+                // the panel's own columns now hold T e_r; phase U must leave them alone (their shadow is zeroed below)
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (k == st) {
+#pragma unroll
+                        for (int e = 0; e < 2; ++e)
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) a[8 * k + c][e] = t[e][c];
+                    }
+            }
+            // ---- shadow copy of this warp's tile (its OLD values are what phase U multiplies): conflict-free 16-byte stores
+#pragma unroll
+            for (int c = 0; c < 32; ++c) Sw[c * 32 + lane] = make_double2(a[c][0], a[c][1]);
+            if (owner) {
+#pragma unroll
+                for (int c = 0; c < 8; ++c) Sw[(8 * st + c) * 32 + lane] = make_double2(0.0, 0.0);
+            }
+            __syncthreads(); // B1: Z, R, sing of this panel visible to both warps (and the shadow to this warp)
+
+            if (sh.sing[buf]) { singular = true; ++gp; break; }
+            int Rv[FR_NB];
+            {
+                const int4 r0 = *reinterpret_cast<const int4 *>(&sh.R[buf][0]);
+                const int4 r1 = *reinterpret_cast<const int4 *>(&sh.R[buf][4]);
+                Rv[0] = r0.x; Rv[1] = r0.y; Rv[2] = r0.z; Rv[3] = r0.w;
+                Rv[4] = r1.x; Rv[5] = r1.y; Rv[6] = r1.z; Rv[7] = r1.w;
+            }
+#pragma unroll
+            for (int b = 0; b < FR_NB; ++b) {
+                if (lane == (Rv[b] >> 1)) usedmask |= 1u << (Rv[b] & 1);
+                if (w == 0 && lane == b) { sh.rho[FR_NB * pnl + b] = Rv[b]; sh.rhoinv[Rv[b]] = FR_NB * pnl + b; }
+            }
+
+            // ---- phase U: rank-8 update  a[:, c] += Z[:, b] * W_old[r_b, c]  of this lane's 2 x 32 tile
+#pragma unroll
+            for (int b = 0; b < FR_NB; ++b) {
+                const double2 z = *reinterpret_cast<const double2 *>(&sh.Z[buf][b][2 * lane]);
+                const double *row = &sh.S[w][0][Rv[b]]; // W_old[r_b, local column c] at row[64 c] (uniform address)
+#pragma unroll
+                for (int c = 0; c < 32; ++c) {
+                    const double rv = row[64 * c];
+                    a[c][0] = fma(z.x, rv, a[c][0]);
+                    a[c][1] = fma(z.y, rv, a[c][1]);
+                }
+            }
+            __syncwarp(); // every lane is done with the shadow before the next panel overwrites it
+        }
+
+        __syncthreads(); // rho / rhoinv complete and visible
+        double *out = Minv + (size_t)cell * n * n;
+        if (singular) {
+            if (threadIdx.x == 0) atomicMin(info, cell + 1);
+            for (int e = threadIdx.x; e < n * n; e += W2_THREADS) out[e] = 0.0;
+            __syncthreads();
+            continue;
+        }
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]
+        const int ro0 = sh.rhoinv[2 * lane], ro1 = sh.rhoinv[2 * lane + 1];
+#pragma unroll
+        for (int c = 0; c < 32; ++c) {
+            double *col = out + (size_t)sh.rho[32 * w + c] * n;
+            col[ro0] = a[c][0];
+            col[ro1] = a[c][1];
         }
     }
 }
@@ -448,7 +658,18 @@ int launch_factor(oci_ctx *ctx)
     const int n = ctx->n;
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream)); // 0x7f7f7f7f = "none"
-    if (ctx->opt_factor_kernel == 1 && n % 64 == 0 && n <= 256) {
+    if (ctx->opt_factor_kernel == 1 && n == 64) {
+        int per_sm = 0;
+        const size_t smem = sizeof(W2Shared);
+        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_w2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_w2_kernel, W2_THREADS, smem));
+        int grid = (per_sm < 1 ? 1 : per_sm) * ctx->num_sms;
+        if (grid > ctx->J) grid = ctx->J;
+        factor_w2_kernel<<<grid, W2_THREADS, smem, ctx->stream>>>(P, ctx->Minv, ctx->info);
+        OCI_CUDA_TRY(ctx, cudaGetLastError());
+        return 1;
+    }
+    if (ctx->opt_factor_kernel >= 1 && n % 64 == 0 && n <= 256) { // 2: the 8-warp kernel also for n = 64
         switch (n / 64) {
         case 1: return launch_factor_reg<1>(ctx, P);
         case 2: return launch_factor_reg<2>(ctx, P);
