@@ -219,3 +219,86 @@ def test_max_iters_reached_without_convergence():
     assert (it_g, conv_g) == (13, 0)
     o.factor(); o.const_rhs(); o.oci_iterate(13)
     assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times (production kernels, check_every = 8).
+# The oracle runs the whole problem (factor + a few iterations: tens of seconds of host time in total), so every
+# cell of every iterate is compared element by element; nothing is sampled from the CUDA path.
+# ---------------------------------------------------------------------------------------------------------------
+FULL_CASES = [
+    ("cfg2", lambda: W.config2(dt=0.01), 4),
+    ("cfg3", lambda: W.config3(), 3),
+    ("cfg4", lambda: W.config4(), 3),
+    ("cfg4b", lambda: W.config4(v=1000.0), 3),
+    ("cfg5@1e-2", lambda: W.config5(dt=1e-2), 3),
+    ("cfg5@1e-4", lambda: W.config5(dt=1e-4), 2),
+]
+
+
+@pytest.mark.parametrize("name,make,n_it", FULL_CASES, ids=[c[0] for c in FULL_CASES])
+def test_full_size_per_iteration_parity(name, make, n_it):
+    p = make()
+    s, o = _solver(p), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    for l in range(n_it):
+        s.iterate(1)
+        o.oci_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"{name}: OCI iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+    # the factors themselves, on cells spread over the slab (first, last, tile boundaries, random)
+    rng = np.random.default_rng(7)
+    for j in sorted({0, 1, p.J // 2, p.J - 2, p.J - 1, *rng.integers(0, p.J, 3).tolist()}):
+        A = o.assemble_cell(j)
+        assert np.array_equal(s.debug_matrix(j), A)
+        assert np.max(np.abs(A @ s.debug_inverse(j) - np.eye(p.n))) < 1e-12 * np.linalg.cond(A)
+
+
+@pytest.mark.parametrize("name,make", [("cfg2", lambda: W.config2(dt=0.01)), ("cfg5@1e-3", lambda: W.config5(dt=1e-3)),
+                                        ("cfg4", lambda: W.config4())], ids=["cfg2", "cfg5@1e-3", "cfg4"])
+def test_full_size_converged_step_parity(name, make):
+    """One converged time step exactly as bench.py runs it (check_every = 8, device-side stop): iteration count equal
+    to the oracle's natural count, converged phi and the state handed to the next step within 1e-9; same for SI."""
+    p = make()
+    s, o = _solver(p), _oracle(p)
+    it_g, conv_g, _ = s.step(tol=p.tol, max_iters=4000, check_every=8)
+    it_o, _ = o.oci_step(tol=p.tol, max_iters=4000)
+    assert it_g == conv_g == it_o
+    assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+    assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+    s2, o2 = _solver(p), _oracle(p)
+    it_g2, conv_g2, _ = s2.si_step(tol=p.tol, max_iters=4000, check_every=8)
+    it_o2, _ = o2.si_step(tol=p.tol, max_iters=4000)
+    assert it_g2 == conv_g2 == it_o2
+    assert rel(s2.scalar_flux().cpu().numpy(), o2.phi) < TOL_PHI
+
+
+def test_full_size_si_per_iteration_parity_cfg5():
+    p = W.config5(dt=1e-2)
+    s, o = _solver(p), _oracle(p)
+    for l in range(3):
+        s.si_iterate(1)
+        o.si_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"SI iteration {l + 1}"
+
+
+@pytest.mark.parametrize("lanes", [4, 16])
+def test_si_lane_groupings_agree(lanes):
+    p = W.random_problem(8, 150, 8, 4, bc_left=1, bc_right=2)
+    s, o = _solver(p, options={"si_lanes": lanes}), _oracle(p)
+    for l in range(3):
+        s.si_iterate(1)
+        o.si_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+def test_factor_kernels_agree_n64():
+    """n = 64: the two-warp kernel (default) and the eight-warp cluster-capable kernel give the same inverse to rounding."""
+    p = W.config5(J=300, dt=1e-3)
+    a, b = _solver(p), _solver(p, options={"factor_kernel": 2})
+    assert a.factor() == 0 and b.factor() == 0
+    for j in (0, 149, 299):
+        A = _oracle(p).assemble_cell(j)
+        for s in (a, b):
+            assert np.max(np.abs(A @ s.debug_inverse(j) - np.eye(64))) < 1e-12 * np.linalg.cond(A)
