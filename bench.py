@@ -46,9 +46,13 @@ CHECK_EVERY = 8
 MAX_ITERS = 4000
 METRIC = "oci_cell_solves_per_s"
 UNIT = "cell-solves/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one oci_iterate_stream_kernel launch on this workload, from the
-# `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one oci_iterate_wpc_kernel<2,0> launch on this workload, from the
+# `ncu --set full` capture summarised in profiles/r01_c_ncu_full.md (2.214780 GB read + 37.87 MB written).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 2252651360
+# same for one factor launch (factor_w2_kernel): 8.8 MB read + 2.097 GB written
+NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2105848448
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
+                                                    # .sum.peak_sustained = 64 per SM) x 2 flop x clocks.max.sm
 
 
 def measured_peaks():
@@ -69,7 +73,7 @@ def algorithmic_bytes_per_cell_solve(n: int, G: int) -> int:
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
@@ -81,7 +85,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -276,19 +280,31 @@ def run_ours(args):
     launch_ms = kernel_ms_total / max(iters_total, 1)
     alg_bytes = algorithmic_bytes_per_cell_solve(n, G) * J
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "oci_iterate_stream_kernel", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "hbm", "kernel": "oci_iterate_wpc_kernel<2,0>", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": launch_ms,
                 "kernel_share_of_step": kernel_ms_total / ms_total}
+    factor_ms = statistics.mean(x for d in per_dt.values() for x in d["factor_ms"])
+    factor_tf = 2.0 * n ** 3 * J / (factor_ms * 1e-3) / 1e12
+    roofline_factor = {"bound": "alu", "kernel": "factor_w2_kernel", "achieved": factor_tf, "peak": FP64_PEAK_TFLOPS,
+                       "unit": "TFLOP/s", "frac": factor_tf / FP64_PEAK_TFLOPS,
+                       "traffic": NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH,
+                       "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md section 7)",
+                       "flops_per_launch": 2.0 * n ** 3 * J, "avg_launch_ms": factor_ms,
+                       "kernel_share_of_step": factor_ms * K / ms_total}
 
     # ---- CPU oracle on the same workload (bounded sample), rank 0, N = 1 only ---------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         sample = p.head(args.cpu_cells)
-        solves, secs, cpu_dt, cores = oracle_pass(sample, SWEEP)
+        solves = secs = 0.0
+        passes = 0
+        while secs < args.cpu_seconds and passes < 64:   # bounded: about 10-30 s of host work
+            s_, t_, cpu_dt, cores = oracle_pass(sample, SWEEP)
+            solves += s_; secs += t_; passes += 1
         cpu = {"value": solves / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {sample.J} of {J} cells of config 5, one converged time step at each dt of {SWEEP} "
-                         f"(factor + iterate + advance), {secs:.1f} s",
+               "sample": f"first {sample.J} of {J} cells of config 5, {passes} pass(es) of one converged time step at each "
+                         f"dt of {SWEEP} (factor + iterate + advance), {secs:.1f} s",
                "iters": [d["iters"] for d in cpu_dt]}
 
     table = []
@@ -312,6 +328,7 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes},
         "gpu_launches": int(launches),
         "roofline": roofline,
+        "roofline_factor": roofline_factor,
         "cpu_baseline": cpu,
         "oci_vs_si": table,
         "max_abs_phi_oci_minus_si": diff,
@@ -328,7 +345,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--cpu-cells", type=int, default=32768, help="cells of the cpu_baseline sample")
+    ap.add_argument("--cpu-cells", type=int, default=65536, help="cells of the cpu_baseline sample")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="minimum host time spent on the cpu_baseline sample")
     ap.add_argument("--ref-cells", type=int, default=8192, help="cells per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-si", action="store_true", help="skip the SI comparator leg (profiling runs)")

@@ -89,6 +89,9 @@ size_t carve(oci_ctx *c, unsigned char *base, int J, int N, int G, int num_sms, 
     const size_t GNpad = (GN + 15) / 16 * 16; // room for any "si_lanes" grouping (4, 8, 16)
     t->si_T2sw = cv.take<double>((size_t)J * GNpad * 4);
     t->si_bsw = cv.take<double>((size_t)J * GNpad * 2);
+    t->st_LinvT = cv.take<double>((size_t)J * GN * 16);
+    t->st_Wg = cv.take<double>((size_t)J * G * 16);
+    t->st_Cinv = cv.take<double>((size_t)J * 16 * G * G);
     t->resid_inf = cv.take<unsigned long long>(OCI_RESID_CAP);
     t->resid_l2 = cv.take<double>(OCI_RESID_CAP);
     t->ctrl = cv.take<int>(4);
@@ -366,6 +369,12 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     else if (!strcmp(key, "factor_kernel")) ctx->opt_factor_kernel = (int)value;
     else if (!strcmp(key, "use_graph")) ctx->opt_use_graph = (int)value;
     else if (!strcmp(key, "refactor_every_step")) ctx->opt_refactor_every_step = (int)value;
+    else if (!strcmp(key, "solve_mode")) {
+        if (value != 0 && value != 1) return -3;
+        if (value == 1 && !st_supported(ctx)) return OCI_E_UNSUPPORTED;
+        if ((int)value != ctx->opt_solve_mode) ctx->factored = false;
+        ctx->opt_solve_mode = (int)value;
+    }
     else if (!strcmp(key, "si_lanes")) { ctx->opt_si_lanes = (int)value; ctx->si_valid = false; }
     else return -2;
     return 0;
@@ -441,7 +450,7 @@ int oci_factor(oci_ctx *ctx)
     if (!ctx) return -1;
     if (ctx->factored) return 0;
     OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-    int r = launch_factor(ctx);
+    int r = ctx->opt_solve_mode == 1 ? launch_st_factor(ctx) : launch_factor(ctx);
     if (r < 0) return r;
     OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     int info = 0;
@@ -554,6 +563,7 @@ int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host)
     if (cell < 0 || cell >= ctx->J) return -2;
     if (!Ainv_host) return -3;
     if (!ctx->factored) return OCI_E_STATE;
+    if (ctx->opt_solve_mode == 1) return OCI_E_UNSUPPORTED; // the structured path never forms A_j^{-1}
     const size_t n = ctx->n;
     std::vector<double> tmp(n * n);
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(tmp.data(), ctx->Minv + (size_t)cell * n * n, sizeof(double) * n * n,

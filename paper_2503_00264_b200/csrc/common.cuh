@@ -49,6 +49,10 @@ struct oci_ctx {
     double *si_in;      // [J][G*N][2]    incident edge flux of cell j found by the sweep
     double *si_T2sw;    // [ceil(GN/lpc)][J][lpc][2][2]  incident -> outgoing 2x2 map, sweep order (si.cu sweep_index)
     double *si_bsw;     // [ceil(GN/lpc)][J][lpc][2]     outgoing entries of si_base, sweep order
+    // structured cell solve ("solve_mode" = 1; structured.cu)
+    double *st_LinvT;   // [J][16][G*N]   L_{c,j,g,m}^-1, ordinate-fastest
+    double *st_Wg;      // [J][G][16]     sum_m w_m L^-1_{j,g,m}
+    double *st_Cinv;    // [J][4G(col)][4G(row)]  (I - V^T D^-1 U)^-1, column-major per cell
     // residual history (device) + pinned host mirror
     unsigned long long *resid_inf; // [OCI_RESID_CAP] bit pattern of a non-negative double
     double *resid_l2;              // [OCI_RESID_CAP] sum of squares
@@ -62,7 +66,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph, opt_refactor_every_step, opt_si_lanes;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph, opt_refactor_every_step, opt_si_lanes, opt_solve_mode;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];
@@ -135,6 +139,9 @@ int launch_advance(oci_ctx *ctx);
 int launch_seed_iterate(oci_ctx *ctx);
 int launch_scalar_flux(oci_ctx *ctx, const double *psi, double *phi);
 int launch_si_setup(oci_ctx *ctx);
+bool st_supported(const oci_ctx *ctx);
+int launch_st_factor(oci_ctx *ctx);
+int launch_st_iteration(oci_ctx *ctx, const struct IterParams &P, bool want_l2);
 int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 
 #ifdef __CUDACC__
@@ -257,4 +264,42 @@ __device__ __forceinline__ double lc_entry(int p, int pp, double dx, double sig,
     default: return 0.0;
     }
 }
+// ---- 4x4 inverse by Gauss-Jordan with partial pivoting, fully unrolled (registers only) ---------------------
+__device__ __forceinline__ void inv4(double (&a)[4][4], double (&b)[4][4])
+{
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) b[i][j] = (i == j) ? 1.0 : 0.0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        int p = k;
+        double best = fabs(a[k][k]);
+#pragma unroll
+        for (int i = k + 1; i < 4; ++i) {
+            const double t = fabs(a[i][k]);
+            if (t > best) { best = t; p = i; }
+        }
+#pragma unroll
+        for (int i = k + 1; i < 4; ++i)
+            if (p == i) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    double t = a[k][j]; a[k][j] = a[i][j]; a[i][j] = t;
+                    t = b[k][j]; b[k][j] = b[i][j]; b[i][j] = t;
+                }
+            }
+        const double inv = 1.0 / a[k][k];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { a[k][j] *= inv; b[k][j] *= inv; }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (i != k) {
+                const double f = a[i][k];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { a[i][j] = fma(-f, a[k][j], a[i][j]); b[i][j] = fma(-f, b[k][j], b[i][j]); }
+            }
+    }
+}
+
 #endif

@@ -581,7 +581,11 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
     P.resid_inf = ctx->resid_inf + hist_slot;
     P.resid_l2 = ctx->resid_l2 + hist_slot;
     const bool wpc_ok = ctx->n == 64 || ctx->n == 128 || ctx->n == 256;
-    if (ctx->opt_iterate_kernel == 1 && wpc_ok) {
+    if (ctx->opt_solve_mode == 1) {
+        P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
+        const int r = launch_st_iteration(ctx, P, want_l2);
+        if (r < 0) return r;
+    } else if (ctx->opt_iterate_kernel == 1 && wpc_ok) {
         const int n = ctx->n;
         const size_t fixed = (size_t)(2 * WPC_MAX_STAGES + 2 * WPC_VEC_SLOTS) * 8 + (size_t)(2 * ctx->N) * 8 + 256 +
                              (size_t)WPC_VEC_SLOTS * ((2 * WPC_WARPS + 2) * n) * 8 + 128;

@@ -16,44 +16,6 @@
 
 namespace {
 
-// ---- 4x4 inverse by Gauss-Jordan with partial pivoting, fully unrolled (registers only) ---------------------
-__device__ __forceinline__ void inv4(double (&a)[4][4], double (&b)[4][4])
-{
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) b[i][j] = (i == j) ? 1.0 : 0.0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        int p = k;
-        double best = fabs(a[k][k]);
-#pragma unroll
-        for (int i = k + 1; i < 4; ++i) {
-            const double t = fabs(a[i][k]);
-            if (t > best) { best = t; p = i; }
-        }
-#pragma unroll
-        for (int i = k + 1; i < 4; ++i)
-            if (p == i) {
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    double t = a[k][j]; a[k][j] = a[i][j]; a[i][j] = t;
-                    t = b[k][j]; b[k][j] = b[i][j]; b[i][j] = t;
-                }
-            }
-        const double inv = 1.0 / a[k][k];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { a[k][j] *= inv; b[k][j] *= inv; }
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-            if (i != k) {
-                const double f = a[i][k];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) { a[i][j] = fma(-f, a[k][j], a[i][j]); b[i][j] = fma(-f, b[k][j], b[i][j]); }
-            }
-    }
-}
-
 // Sweep-order record index of (cell j, ordinate gm): chains are grouped `lpc` to a CTA; within a CTA's slab the
 // records of one sweep step jj (cell jj for mu > 0, cell J-1-jj for mu < 0) of its lpc chains are contiguous, so a
 // tile of consecutive sweep steps is ONE contiguous block that a single bulk copy brings into shared memory.

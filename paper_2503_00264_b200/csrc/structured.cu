@@ -1,0 +1,291 @@
+// structured.cu -- SURVEY.md section 8(f), NEXT row f1: the structured cell solve ("solve_mode" = 1).
+//
+// The paper stores A_j dense although only 25 % of it is non-zero and names sparse cell blocks as future work
+// (Eq. 41). By Eq. 8a-b, 10 and 40b
+//     A_j = D - U V^T,   D = blockdiag_{(g,m)} L_{c,j,g,m}  (4 x 4 blocks, Eq. 8b),
+//     V^T psi = phi      (phi[g][p] = sum_m w_m psi[g][m][p], Eq. 44),   (U phi)[g][m][p] = dx_j/4 sum_g' K_j[g][g'] phi[g'][p],
+// so, exactly (Sherman-Morrison-Woodbury), the cell solve A_j x = b of Eq. 7 is
+//     z = D^-1 b;   phi_z = V^T z;   y = C^-1 phi_z,  C = I - V^T D^-1 U  (4G x 4G);   x = z + D^-1 U y,
+// and y = V^T x is the new scalar flux itself. Same iteration, same fixed point, same oracle (parity to
+// 1e-11: cond(D), cond(C) <= ~1e3), but 4n + 16 G^2 doubles of factors per cell-solve instead of n^2.
+//   st_setup   (once per dt): L^-1 of every 4 x 4 block (partial pivoting), W_g = sum_m w_m L^-1_{g,m}
+//   st_cap     (once per dt): C = I - dx/4 (K (x) 1) W assembled on chip, inverted with partial pivoting
+//   st_iterate (every iteration): a4-a7 fused, one thread per (cell, g, m)
+#include "common.cuh"
+#include <limits.h>
+
+namespace {
+
+// ---- once per (problem, dt): LinvT[j][k][gm] = (L_{c,j,g,m}^-1)[k/4][k%4] (ordinate-fastest, so that the iterate
+// kernel's loads are contiguous across its threads) and Wg[j][g][16] = sum_m w_m L^-1_{j,g,m}. One thread per (j,g).
+__global__ void st_setup_kernel(ProblemView P, double *__restrict__ LinvT, double *__restrict__ Wg)
+{
+    const size_t total = (size_t)P.J * P.G;
+    const int GN = P.G * P.N;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+        const int g = (int)(e % P.G);
+        const size_t j = e / P.G;
+        const double dx = P.dx[j], sig = P.sigma_t[e], v = P.v[g];
+        double acc[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) acc[k] = 0.0;
+        for (int m = 0; m < P.N; ++m) {
+            const double mu = P.mu[m], wm = P.w[m];
+            double a[4][4], b[4][4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p)
+#pragma unroll
+                for (int pp = 0; pp < 4; ++pp) a[p][pp] = lc_entry(p, pp, dx, sig, v, P.dt, mu);
+            inv4(a, b);
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                LinvT[(j * 16 + k) * GN + g * P.N + m] = b[k >> 2][k & 3];
+                acc[k] = fma(wm, b[k >> 2][k & 3], acc[k]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 16; ++k) Wg[e * 16 + k] = acc[k];
+    }
+}
+
+// C[(g,p)][(g',p')] = delta - (dx/4 K[g][g']) W_g[p][p']
+__device__ __forceinline__ double cap_entry(const ProblemView &P, const double *__restrict__ Wg, size_t cell, int i, int c)
+{
+    const int g = i >> 2, p = i & 3, gc = c >> 2, pc = c & 3;
+    const double k4 = P.dx[cell] * 0.25 * P.transfer[(cell * P.G + g) * P.G + gc];
+    return (i == c ? 1.0 : 0.0) - k4 * Wg[(cell * P.G + g) * 16 + p * 4 + pc];
+}
+
+// ---- once per (problem, dt): C^-1 by Gauss-Jordan with partial pivoting (first maximal |entry|), one warp per cell,
+// lane = row (4G <= 32), the matrix in shared memory. Stored column-major: Cinv[j][col][row].
+constexpr int CAP_WARPS = 4;
+constexpr int CAP_LD = 33;
+
+__global__ void __launch_bounds__(CAP_WARPS * 32) st_cap_kernel(ProblemView P, const double *__restrict__ Wg,
+                                                                double *__restrict__ Cinv, int *info)
+{
+    __shared__ double Wsm[CAP_WARPS][32][CAP_LD];
+    __shared__ int rho_s[CAP_WARPS][32], rhoinv_s[CAP_WARPS][32];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    const int dim = 4 * P.G;
+    double(*W)[CAP_LD] = Wsm[wp];
+    int *rho = rho_s[wp], *rhoinv = rhoinv_s[wp];
+    const unsigned FULL = 0xffffffffu;
+    for (size_t cell = (size_t)blockIdx.x * CAP_WARPS + wp; cell < (size_t)P.J; cell += (size_t)gridDim.x * CAP_WARPS) {
+        for (int i = 0; i < dim; ++i)
+            if (lane < dim) W[i][lane] = cap_entry(P, Wg, cell, i, lane);
+        __syncwarp();
+        bool used = false, singular = false;
+        for (int k = 0; k < dim; ++k) {
+            const double v = lane < dim ? W[lane][k] : 0.0;
+            double cand = (lane < dim && !used) ? fabs(v) : -1.0;
+            if (!(cand == cand)) cand = __longlong_as_double(0x7ff0000000000000LL); // NaN -> +inf: found and flagged
+            int ci = lane;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double oc = __shfl_xor_sync(FULL, cand, o);
+                const int oi = __shfl_xor_sync(FULL, ci, o);
+                if (oc > cand || (oc == cand && oi < ci)) { cand = oc; ci = oi; }
+            }
+            if (!(cand > 0.0) || cand > 1.7e308) { singular = true; break; } // warp-uniform
+            const int r = ci;
+            const double inv = 1.0 / __shfl_sync(FULL, v, r);
+            const double pr = lane < dim ? (lane == k ? 1.0 : W[r][lane]) * inv : 0.0;
+            for (int i = 0; i < dim; ++i) {
+                const double f = __shfl_sync(FULL, v, i);
+                if (lane < dim) W[i][lane] = (i == r) ? pr : fma(-f, pr, lane == k ? 0.0 : W[i][lane]);
+            }
+            if (lane == r) used = true;
+            if (lane == 0) { rho[k] = r; rhoinv[r] = k; }
+            __syncwarp();
+        }
+        double *out = Cinv + cell * dim * dim;
+        if (singular) {
+            if (lane == 0) atomicMin(info, (int)cell + 1);
+            for (int e = lane; e < dim * dim; e += 32) out[e] = 0.0;
+        } else { // Cinv[kappa][rho_j] = W[rho_kappa][j]: un-scrambles the implicit row exchange
+            for (int jc = 0; jc < dim; ++jc)
+                if (lane < dim) out[(size_t)rho[jc] * dim + rhoinv[lane]] = W[lane][jc];
+        }
+        __syncwarp();
+    }
+}
+
+// ---- every iteration: a4 (gather + RHS), a5 (structured solve), a6 (phi), a7 (residual), one thread per (cell, g, m).
+// A CTA works on CPB = 256 / (G N) consecutive cells at a time. Loads are contiguous across the threads of a cell
+// (c_j and Psi: 32 bytes per thread; LinvT: ordinate-fastest; Cinv: column-major, one row per thread).
+constexpr int ST_THREADS = 256;
+
+struct StParams {
+    const double *LinvT, *Cinv, *dx, *transfer;
+};
+
+template <bool WANT_L2>
+__global__ void __launch_bounds__(ST_THREADS) st_iterate_kernel(const IterParams P, const StParams S)
+{
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
+    extern __shared__ __align__(16) double st_smem[];
+    const int N = P.N, G = P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
+    const int CPB = ST_THREADS / GN;
+    double *mu_s = st_smem;                 // [N]
+    double *w_s = mu_s + N;                 // [N]
+    double *wz = w_s + N;                   // [CPB][GN][4]   w_m z
+    double *phiz = wz + (size_t)CPB * GN * 4; // [CPB][4G]
+    double *ys = phiz + (size_t)CPB * G4;   // [CPB][4G]
+    double *ss = ys + (size_t)CPB * G4;     // [CPB][4G]
+    const int tid = threadIdx.x, lane = tid & 31;
+    for (int i = tid; i < N; i += ST_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    __syncthreads();
+
+    const int a = tid / GN, gm = tid - a * GN, g = gm / N, m = gm - g * N;
+    const bool lane_on = tid < CPB * GN;
+    double rmax = 0.0, l2 = 0.0;
+
+    for (int base = blockIdx.x * CPB; base < J; base += gridDim.x * CPB) {
+        const int j = base + a;
+        const bool on = lane_on && j < J;
+        double L[16], z[4];
+        if (on) {
+            const double2 c01 = *reinterpret_cast<const double2 *>(P.c + (size_t)j * n + gm * 4);
+            const double2 c23 = *reinterpret_cast<const double2 *>(P.c + (size_t)j * n + gm * 4 + 2);
+            double b[4] = {c01.x, c01.y, c23.x, c23.y};
+            // ---- a4: incident edge fluxes from Psi^(l) (Eq. 9c-d; closures Eq. 5a-b)
+            const double mu = mu_s[m];
+            const double *self = P.psi_old + (size_t)j * n;
+            if (mu > 0.0) { // rows (k,L), (k+1/2,L): upstream = (j-1, R)
+                double v0, v1;
+                if (j > 0) { v0 = (self - n)[gm * 4 + 1]; v1 = (self - n)[gm * 4 + 3]; }
+                else if (P.bc_left == OCI_BC_REFLECTIVE) {
+                    v0 = self[(g * N + (N - 1 - m)) * 4 + 0]; v1 = self[(g * N + (N - 1 - m)) * 4 + 2];
+                } else if (P.bc_left == OCI_BC_PRESCRIBED) { v0 = P.inc_left[gm * 2]; v1 = P.inc_left[gm * 2 + 1]; }
+                else { v0 = 0.0; v1 = 0.0; }
+                b[0] += mu * v0;
+                b[2] += mu * v1;
+            } else {        // rows (k,R), (k+1/2,R): upstream = (j+1, L)
+                double v0, v1;
+                if (j < J - 1) { v0 = (self + n)[gm * 4 + 0]; v1 = (self + n)[gm * 4 + 2]; }
+                else if (P.bc_right == OCI_BC_REFLECTIVE) {
+                    v0 = self[(g * N + (N - 1 - m)) * 4 + 1]; v1 = self[(g * N + (N - 1 - m)) * 4 + 3];
+                } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = P.inc_right[gm * 2]; v1 = P.inc_right[gm * 2 + 1]; }
+                else { v0 = 0.0; v1 = 0.0; }
+                b[1] += -mu * v0;
+                b[3] += -mu * v1;
+            }
+            // ---- z = D^-1 b
+            const double *Lp = S.LinvT + (size_t)j * 16 * GN + gm;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) L[k] = Lp[(size_t)k * GN];
+            const double wm = w_s[m];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                z[p] = fma(L[p * 4 + 3], b[3], fma(L[p * 4 + 2], b[2], fma(L[p * 4 + 1], b[1], L[p * 4] * b[0])));
+                wz[(size_t)tid * 4 + p] = wm * z[p];
+            }
+        }
+        __syncthreads();
+        // ---- phi_z = V^T z, y = C^-1 phi_z = phi^(l+1) (a6), residual (a7), s = dx/4 K y: one (cell, g, p) row per
+        // thread-iteration (4G rows per cell; 4G > G N when N = 2, hence the loops)
+        const int rows = CPB * G4;
+        for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4;
+            if (base + a2 < J) {
+                const int g2 = r2 >> 2, p2 = r2 & 3;
+                const double *src = wz + ((size_t)a2 * GN + g2 * N) * 4 + p2;
+                double acc = 0.0;
+                for (int mm = 0; mm < N; ++mm) acc += src[mm * 4];
+                phiz[t2] = acc;
+            }
+        }
+        __syncthreads();
+        for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = base + a2;
+            if (j2 < J) {
+                const double *Cp = S.Cinv + (size_t)j2 * G4 * G4 + r2;
+                const double *pz = phiz + a2 * G4;
+                double y = 0.0;
+                for (int cc = 0; cc < G4; ++cc) y = fma(Cp[(size_t)cc * G4], pz[cc], y);
+                ys[t2] = y;
+                double *ph = P.phi + (size_t)j2 * G4 + r2;
+                const double d = fabs(y - *ph);
+                *ph = y;
+                rmax = (d > rmax || !(d == d)) ? d : rmax;
+            }
+        }
+        __syncthreads();
+        for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = base + a2;
+            if (j2 < J) {
+                const int g2 = r2 >> 2, p2 = r2 & 3;
+                const double *Kr = S.transfer + ((size_t)j2 * G + g2) * G;
+                const double *yy = ys + a2 * G4 + p2;
+                double acc = 0.0;
+                for (int gc = 0; gc < G; ++gc) acc = fma(Kr[gc], yy[gc * 4], acc);
+                ss[t2] = S.dx[j2] * 0.25 * acc;
+            }
+        }
+        __syncthreads();
+        // ---- x = z + D^-1 U y
+        if (on) {
+            const double *sv = ss + a * G4 + g * 4;
+            const double s0 = sv[0], s1 = sv[1], s2 = sv[2], s3 = sv[3];
+            double x[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p)
+                x[p] = fma(L[p * 4 + 3], s3, fma(L[p * 4 + 2], s2, fma(L[p * 4 + 1], s1, fma(L[p * 4], s0, z[p]))));
+            double *out = P.psi_new + (size_t)j * n + gm * 4;
+            if (WANT_L2) {
+                const double *old = P.psi_old + (size_t)j * n + gm * 4;
+#pragma unroll
+                for (int p = 0; p < 4; ++p) { const double d = x[p] - old[p]; l2 = fma(d, d, l2); }
+            }
+            *reinterpret_cast<double2 *>(out) = make_double2(x[0], x[1]);
+            *reinterpret_cast<double2 *>(out + 2) = make_double2(x[2], x[3]);
+        }
+        // wz / phiz / ys / ss are rewritten only after the next iteration's first barrier sequence; wz is written
+        // before that barrier by threads that may still be read by slower ones here -> one more barrier
+        __syncthreads();
+    }
+    rmax = warp_max(rmax);
+    if (lane == 0) atomicMax(P.resid_inf, resid_bits(rmax));
+    if (WANT_L2) {
+        l2 = warp_sum(l2);
+        if (lane == 0) atomicAdd(P.resid_l2, l2);
+    }
+}
+
+} // namespace
+
+bool st_supported(const oci_ctx *ctx) { return 4 * ctx->G <= 32 && ctx->G * ctx->N <= ST_THREADS; }
+
+// a1 + a2 of the structured path; returns the number of kernels launched
+int launch_st_factor(oci_ctx *ctx)
+{
+    if (!st_supported(ctx)) return OCI_E_UNSUPPORTED;
+    ProblemView P = make_view(ctx);
+    OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream));
+    const size_t total = (size_t)ctx->J * ctx->G;
+    size_t g1 = (total + 127) / 128;
+    if (g1 > (size_t)ctx->num_sms * 16) g1 = (size_t)ctx->num_sms * 16;
+    st_setup_kernel<<<(int)g1, 128, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    size_t g2 = ((size_t)ctx->J + CAP_WARPS - 1) / CAP_WARPS;
+    if (g2 > (size_t)ctx->num_sms * 4) g2 = (size_t)ctx->num_sms * 4;
+    st_cap_kernel<<<(int)g2, CAP_WARPS * 32, 0, ctx->stream>>>(P, ctx->st_Wg, ctx->st_Cinv, ctx->info);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 2;
+}
+
+int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
+{
+    StParams S;
+    S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
+    const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
+    const size_t smem = sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 + (size_t)3 * CPB * G4);
+    int grid = (ctx->J + CPB - 1) / CPB;
+    if (grid > ctx->num_sms * 8) grid = ctx->num_sms * 8;
+    if (want_l2) st_iterate_kernel<true><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);
+    else st_iterate_kernel<false><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}

@@ -302,3 +302,75 @@ def test_factor_kernels_agree_n64():
         A = _oracle(p).assemble_cell(j)
         for s in (a, b):
             assert np.max(np.abs(A @ s.debug_inverse(j) - np.eye(64))) < 1e-12 * np.linalg.cond(A)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# structured cell solve ("solve_mode" = 1). Same oracle, same tolerances.
+# ---------------------------------------------------------------------------------------------------------------
+ST = {"solve_mode": 1}
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
+def test_structured_per_iteration_parity(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p, options=ST), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    for l in range(6):
+        s.iterate(1)
+        o.oci_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+    s.iterate(7)
+    o.oci_iterate(7)
+    assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+@pytest.mark.parametrize("name,make,n_it", FULL_CASES, ids=[c[0] for c in FULL_CASES])
+def test_structured_full_size_parity(name, make, n_it):
+    p = make()
+    s, o = _solver(p, options=ST), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    for l in range(n_it):
+        s.iterate(1)
+        o.oci_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"{name}: iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("k", [1, 5])
+def test_structured_step_loop_matches_oracle(rule, k):
+    p = W.random_problem(33, 61, 4, 2, bc_left=1, bc_right=2, dt=0.05)
+    s, o = _solver(p, options=ST), _oracle(p)
+    for step in range(3):
+        it_g, conv_g, _ = s.step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
+        it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule)
+        assert it_g == conv_g == it_o, f"step {step}"
+        np.testing.assert_allclose(s.residual_history(kind=rule), hist_o, rtol=1e-6, atol=1e-15)
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+def test_structured_and_dense_paths_agree_on_a_converged_config5_step():
+    p = W.config5(dt=1e-1)
+    a, b = _solver(p, options=ST), _solver(p)
+    ia, _, _ = a.step(tol=p.tol, max_iters=4000, check_every=8)
+    ib, _, _ = b.step(tol=p.tol, max_iters=4000, check_every=8)
+    assert ia == ib
+    assert rel(a.scalar_flux().cpu().numpy(), b.scalar_flux().cpu().numpy()) < 1e-12
+
+
+def test_structured_mode_switch_refactors_and_flags_singular():
+    p = W.random_problem(21, 12, 4, 1)
+    s = _solver(p)
+    s.factor()
+    s.set_option("solve_mode", 1)
+    with pytest.raises(Exception):
+        s.iterate(1)                 # factors of the other mode: OCI_E_STATE
+    assert s.factor() == 0
+    s.iterate(2)
+    p.sigma_t = p.sigma_t.copy()
+    p.sigma_t[7] = np.nan
+    assert _solver(p, options=ST).factor() == 8
