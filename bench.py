@@ -66,6 +66,12 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def structured_bytes_per_cell_solve(n: int, G: int) -> int:
+    """DESIGN.md section 5 (structured cell solve): L^-1 blocks (32 n) + c (8n) + neighbour edge flux
+    (4n) + Psi write (8n) + C^-1 (128 G^2) + K (8 G^2) + dx (8) + phi read/write (64 G)."""
+    return 52 * n + 136 * G * G + 64 * G + 8
+
+
 def algorithmic_bytes_per_cell_solve(n: int, G: int) -> int:
     """A_j^{-1} (8 n^2) + c (8n) + neighbour edge flux (4n) + index/perm (4n) + Psi write (8n) +
     phi old/new (64 G)."""
@@ -237,6 +243,33 @@ def run_ours(args):
         ms_total = float(t.item())
     value = world * J * iters_total / (ms_total * 1e-3)
 
+    # ---- structured cell solve, same sequence, reported beside (not part of `value`) -----------
+    st = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}", options={"solve_mode": 1})
+    for i in range(Wm):
+        oci_step(i, st)
+    st_iters = 0
+    st_kernel_ms = 0.0
+    st_factor_ms = []
+    barrier()
+    ev0.record()
+    for i in range(Wm, Wm + K):
+        t = time.perf_counter()
+        it, conv, _ = oci_step(i, st)
+        el = (time.perf_counter() - t) * 1e3
+        d = per_dt[SWEEP[i % len(SWEEP)]]
+        d.setdefault("st_iters", []).append(it); d.setdefault("st_ms", []).append(el)
+        st_iters += it
+        st_kernel_ms += st.last_timing(1)[0]
+        st_factor_ms.append(st.last_timing(0)[0])
+    ev1.record()
+    barrier()
+    st_ms_total = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([st_ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        st_ms_total = float(t.item())
+    st_diff = float((oci.scalar_flux() - st.scalar_flux()).abs().max().item())
+
     # ---- SI comparator, same sequence (reported beside, not part of `value`) ----------------------------------
     for i in range(0 if args.no_si else Wm):
         si.set_dt(SWEEP[i % len(SWEEP)]); si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
@@ -293,6 +326,20 @@ def run_ours(args):
                        "flops_per_launch": 2.0 * n ** 3 * J, "avg_launch_ms": factor_ms,
                        "kernel_share_of_step": factor_ms * K / ms_total}
 
+    st_launch_ms = st_kernel_ms / max(st_iters, 1)
+    st_bytes = structured_bytes_per_cell_solve(n, G) * J
+    st_achieved = st_bytes / (st_launch_ms * 1e-3) / 1e9
+    structured = {
+        "what": "SURVEY 8(f) row f1: structured cell solve A_j = D - U V^T (solve_mode = 1), same steps, same stop rule",
+        "value": world * J * st_iters / (st_ms_total * 1e-3), "unit": UNIT, "ms_per_step": st_ms_total / K,
+        "iterations_total": st_iters, "factor_ms": statistics.mean(st_factor_ms),
+        "max_abs_phi_minus_dense_path": st_diff,
+        "roofline": {"bound": "hbm", "kernel": "st_iterate_kernel", "achieved": st_achieved, "peak": peak, "unit": "GB/s",
+                     "frac": st_achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": st_bytes, "avg_launch_ms": st_launch_ms,
+                     "kernel_share_of_step": st_kernel_ms / st_ms_total},
+    }
+
     # ---- CPU oracle on the same workload (bounded sample), rank 0, N = 1 only ---------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -315,6 +362,8 @@ def run_ours(args):
         table.append({"dt": dt, "oci_iters": d["oci_iters"], "si_iters": d.get("si_iters"),
                       "oci_ms_per_step": statistics.mean(d["oci_ms"]), "oci_factor_ms": statistics.mean(d["factor_ms"]),
                       "oci_iter_kernel_ms": statistics.mean(d["iter_kernel_ms"]),
+                      "structured_iters": d.get("st_iters"),
+                      "structured_ms_per_step": statistics.mean(d["st_ms"]) if d.get("st_ms") else None,
                       "si_ms_per_step": statistics.mean(d["si_ms"]) if d.get("si_ms") else None})
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
@@ -329,6 +378,7 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "roofline": roofline,
         "roofline_factor": roofline_factor,
+        "structured": structured,
         "cpu_baseline": cpu,
         "oci_vs_si": table,
         "max_abs_phi_oci_minus_si": diff,

@@ -8,7 +8,7 @@
 //     z = D^-1 b;   phi_z = V^T z;   y = C^-1 phi_z,  C = I - V^T D^-1 U  (4G x 4G);   x = z + D^-1 U y,
 // and y = V^T x is the new scalar flux itself. Same iteration, same fixed point, same oracle (parity to
 // 1e-11: cond(D), cond(C) <= ~1e3), but 4n + 16 G^2 doubles of factors per cell-solve instead of n^2.
-//   st_setup   (once per dt): L^-1 of every 4 x 4 block (partial pivoting), W_g = sum_m w_m L^-1_{g,m}
+//   st_setup   (once per dt): L^-1 of every 4 x 4 block (partial pivoting); st_wsum: W_g = sum_m w_m L^-1_{g,m}
 //   st_cap     (once per dt): C = I - dx/4 (K (x) 1) W assembled on chip, inverted with partial pivoting
 //   st_iterate (every iteration): a4-a7 fused, one thread per (cell, g, m)
 #include "common.cuh"
@@ -17,34 +17,40 @@
 namespace {
 
 // ---- once per (problem, dt): LinvT[j][k][gm] = (L_{c,j,g,m}^-1)[k/4][k%4] (ordinate-fastest, so that the iterate
-// kernel's loads are contiguous across its threads) and Wg[j][g][16] = sum_m w_m L^-1_{j,g,m}. One thread per (j,g).
-__global__ void st_setup_kernel(ProblemView P, double *__restrict__ LinvT, double *__restrict__ Wg)
+// kernel's loads and these stores are contiguous across threads). One thread per (j,g,m).
+__global__ void st_setup_kernel(ProblemView P, double *__restrict__ LinvT)
 {
-    const size_t total = (size_t)P.J * P.G;
     const int GN = P.G * P.N;
+    const size_t total = (size_t)P.J * GN;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
-        const int g = (int)(e % P.G);
-        const size_t j = e / P.G;
-        const double dx = P.dx[j], sig = P.sigma_t[e], v = P.v[g];
-        double acc[16];
+        const int gm = (int)(e % GN), g = gm / P.N, m = gm - g * P.N;
+        const size_t j = e / GN;
+        const double dx = P.dx[j], sig = P.sigma_t[j * P.G + g], v = P.v[g], mu = P.mu[m];
+        double a[4][4], b[4][4];
 #pragma unroll
-        for (int k = 0; k < 16; ++k) acc[k] = 0.0;
-        for (int m = 0; m < P.N; ++m) {
-            const double mu = P.mu[m], wm = P.w[m];
-            double a[4][4], b[4][4];
+        for (int p = 0; p < 4; ++p)
 #pragma unroll
-            for (int p = 0; p < 4; ++p)
+            for (int pp = 0; pp < 4; ++pp) a[p][pp] = lc_entry(p, pp, dx, sig, v, P.dt, mu);
+        inv4(a, b);
 #pragma unroll
-                for (int pp = 0; pp < 4; ++pp) a[p][pp] = lc_entry(p, pp, dx, sig, v, P.dt, mu);
-            inv4(a, b);
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                LinvT[(j * 16 + k) * GN + g * P.N + m] = b[k >> 2][k & 3];
-                acc[k] = fma(wm, b[k >> 2][k & 3], acc[k]);
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 16; ++k) Wg[e * 16 + k] = acc[k];
+        for (int k = 0; k < 16; ++k) LinvT[(j * 16 + k) * GN + gm] = b[k >> 2][k & 3];
+    }
+}
+
+// Wg[j][g][k] = sum_m w_m (L^-1_{j,g,m})[k]. One thread per (j,g,k).
+__global__ void st_wsum_kernel(ProblemView P, const double *__restrict__ LinvT, double *__restrict__ Wg)
+{
+    const int GN = P.G * P.N;
+    const size_t total = (size_t)P.J * P.G * 16;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
+        const int k = (int)(e & 15);
+        const size_t jg = e >> 4;
+        const int g = (int)(jg % P.G);
+        const size_t j = jg / P.G;
+        const double *src = LinvT + (j * 16 + k) * GN + (size_t)g * P.N;
+        double acc = 0.0;
+        for (int m = 0; m < P.N; ++m) acc = fma(P.w[m], src[m], acc);
+        Wg[e] = acc;
     }
 }
 
@@ -120,65 +126,83 @@ struct StParams {
     const double *LinvT, *Cinv, *dx, *transfer;
 };
 
-template <bool WANT_L2>
-__global__ void __launch_bounds__(ST_THREADS) st_iterate_kernel(const IterParams P, const StParams S)
+// GC = G when G is 1, 2, 4 or 8 (the 4G rows of a cell then sit inside one warp, so the three small steps between
+// z and x need only __syncwarp, and for G <= 4 the thread's row of C^-1, its row of K and dx are loaded up front,
+// together with everything else, so that a CTA waits for HBM once); GC = 0: any G, CTA-wide barriers.
+template <bool WANT_L2, int GC>
+__global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterParams P, const StParams S)
 {
     if (stop_reached(P.stop)) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
     extern __shared__ __align__(16) double st_smem[];
-    const int N = P.N, G = P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
+    const int N = P.N, G = GC > 0 ? GC : P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
+    constexpr bool PRE = GC > 0 && GC <= 4;
+    constexpr int GP = PRE ? GC : 1;
     const int CPB = ST_THREADS / GN;
-    double *mu_s = st_smem;                 // [N]
-    double *w_s = mu_s + N;                 // [N]
-    double *wz = w_s + N;                   // [CPB][GN][4]   w_m z
+    double *mu_s = st_smem;                   // [N]
+    double *w_s = mu_s + N;                   // [N]
+    double *wz = w_s + N;                     // [CPB][GN][4]   w_m z
     double *phiz = wz + (size_t)CPB * GN * 4; // [CPB][4G]
-    double *ys = phiz + (size_t)CPB * G4;   // [CPB][4G]
-    double *ss = ys + (size_t)CPB * G4;     // [CPB][4G]
+    double *ys = phiz + (size_t)CPB * G4;     // [CPB][4G]
+    double *ss = ys + (size_t)CPB * G4;       // [CPB][4G]
     const int tid = threadIdx.x, lane = tid & 31;
     for (int i = tid; i < N; i += ST_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
-    __syncthreads();
 
     const int a = tid / GN, gm = tid - a * GN, g = gm / N, m = gm - g * N;
     const bool lane_on = tid < CPB * GN;
+    const int rows = CPB * G4;
     double rmax = 0.0, l2 = 0.0;
+    auto small_sync = [&]() {
+        if (GC > 0) __syncwarp();
+        else __syncthreads();
+    };
 
     for (int base = blockIdx.x * CPB; base < J; base += gridDim.x * CPB) {
         const int j = base + a;
         const bool on = lane_on && j < J;
-        double L[16], z[4];
+        double L[16], z[4], b[4], v0 = 0.0, v1 = 0.0, mu = 1.0;
+        // ---- all global loads of this batch up front
         if (on) {
             const double2 c01 = *reinterpret_cast<const double2 *>(P.c + (size_t)j * n + gm * 4);
             const double2 c23 = *reinterpret_cast<const double2 *>(P.c + (size_t)j * n + gm * 4 + 2);
-            double b[4] = {c01.x, c01.y, c23.x, c23.y};
-            // ---- a4: incident edge fluxes from Psi^(l) (Eq. 9c-d; closures Eq. 5a-b)
-            const double mu = mu_s[m];
+            b[0] = c01.x; b[1] = c01.y; b[2] = c23.x; b[3] = c23.y;
+            mu = P.mu[m];
             const double *self = P.psi_old + (size_t)j * n;
+            // a4: incident edge fluxes from Psi^(l) (Eq. 9c-d; closures Eq. 5a-b)
             if (mu > 0.0) { // rows (k,L), (k+1/2,L): upstream = (j-1, R)
-                double v0, v1;
                 if (j > 0) { v0 = (self - n)[gm * 4 + 1]; v1 = (self - n)[gm * 4 + 3]; }
                 else if (P.bc_left == OCI_BC_REFLECTIVE) {
                     v0 = self[(g * N + (N - 1 - m)) * 4 + 0]; v1 = self[(g * N + (N - 1 - m)) * 4 + 2];
                 } else if (P.bc_left == OCI_BC_PRESCRIBED) { v0 = P.inc_left[gm * 2]; v1 = P.inc_left[gm * 2 + 1]; }
-                else { v0 = 0.0; v1 = 0.0; }
-                b[0] += mu * v0;
-                b[2] += mu * v1;
             } else {        // rows (k,R), (k+1/2,R): upstream = (j+1, L)
-                double v0, v1;
                 if (j < J - 1) { v0 = (self + n)[gm * 4 + 0]; v1 = (self + n)[gm * 4 + 2]; }
                 else if (P.bc_right == OCI_BC_REFLECTIVE) {
                     v0 = self[(g * N + (N - 1 - m)) * 4 + 1]; v1 = self[(g * N + (N - 1 - m)) * 4 + 3];
                 } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = P.inc_right[gm * 2]; v1 = P.inc_right[gm * 2 + 1]; }
-                else { v0 = 0.0; v1 = 0.0; }
-                b[1] += -mu * v0;
-                b[3] += -mu * v1;
             }
-            // ---- z = D^-1 b
             const double *Lp = S.LinvT + (size_t)j * 16 * GN + gm;
 #pragma unroll
             for (int k = 0; k < 16; ++k) L[k] = Lp[(size_t)k * GN];
+        }
+        double Cr[4 * GP], Kr[GP], dxq = 0.0, phi_old = 0.0; // this thread's (first) row of the 4G-system
+        if (PRE && tid < rows && base + tid / G4 < J) {
+            const int a2 = tid / G4, r2 = tid - a2 * G4, j2 = base + a2;
+            const double *Cp = S.Cinv + (size_t)j2 * G4 * G4 + r2;
+#pragma unroll
+            for (int cc = 0; cc < 4 * GP; ++cc) Cr[cc] = Cp[(size_t)cc * G4];
+            const double *Kp = S.transfer + ((size_t)j2 * G + (r2 >> 2)) * G;
+#pragma unroll
+            for (int gc = 0; gc < GP; ++gc) Kr[gc] = Kp[gc];
+            dxq = S.dx[j2] * 0.25;
+            phi_old = P.phi[(size_t)j2 * G4 + r2];
+        }
+        __syncthreads(); // previous batch done with the shared arrays (and mu_s / w_s loaded)
+        if (on) {
+            if (mu > 0.0) { b[0] = fma(mu, v0, b[0]); b[2] = fma(mu, v1, b[2]); }
+            else { b[1] = fma(-mu, v0, b[1]); b[3] = fma(-mu, v1, b[3]); }
             const double wm = w_s[m];
 #pragma unroll
-            for (int p = 0; p < 4; ++p) {
+            for (int p = 0; p < 4; ++p) { // z = D^-1 b
                 z[p] = fma(L[p * 4 + 3], b[3], fma(L[p * 4 + 2], b[2], fma(L[p * 4 + 1], b[1], L[p * 4] * b[0])));
                 wz[(size_t)tid * 4 + p] = wm * z[p];
             }
@@ -186,7 +210,6 @@ __global__ void __launch_bounds__(ST_THREADS) st_iterate_kernel(const IterParams
         __syncthreads();
         // ---- phi_z = V^T z, y = C^-1 phi_z = phi^(l+1) (a6), residual (a7), s = dx/4 K y: one (cell, g, p) row per
         // thread-iteration (4G rows per cell; 4G > G N when N = 2, hence the loops)
-        const int rows = CPB * G4;
         for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
             const int a2 = t2 / G4, r2 = t2 - a2 * G4;
             if (base + a2 < J) {
@@ -197,31 +220,43 @@ __global__ void __launch_bounds__(ST_THREADS) st_iterate_kernel(const IterParams
                 phiz[t2] = acc;
             }
         }
-        __syncthreads();
+        small_sync();
         for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
             const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = base + a2;
             if (j2 < J) {
-                const double *Cp = S.Cinv + (size_t)j2 * G4 * G4 + r2;
                 const double *pz = phiz + a2 * G4;
-                double y = 0.0;
-                for (int cc = 0; cc < G4; ++cc) y = fma(Cp[(size_t)cc * G4], pz[cc], y);
+                double y = 0.0, po;
+                if (PRE && t2 == tid) {
+#pragma unroll
+                    for (int cc = 0; cc < 4 * GP; ++cc) y = fma(Cr[cc], pz[cc], y);
+                    po = phi_old;
+                } else {
+                    const double *Cp = S.Cinv + (size_t)j2 * G4 * G4 + r2;
+                    for (int cc = 0; cc < G4; ++cc) y = fma(Cp[(size_t)cc * G4], pz[cc], y);
+                    po = P.phi[(size_t)j2 * G4 + r2];
+                }
                 ys[t2] = y;
-                double *ph = P.phi + (size_t)j2 * G4 + r2;
-                const double d = fabs(y - *ph);
-                *ph = y;
+                P.phi[(size_t)j2 * G4 + r2] = y;
+                const double d = fabs(y - po);
                 rmax = (d > rmax || !(d == d)) ? d : rmax;
             }
         }
-        __syncthreads();
+        small_sync();
         for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
             const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = base + a2;
             if (j2 < J) {
                 const int g2 = r2 >> 2, p2 = r2 & 3;
-                const double *Kr = S.transfer + ((size_t)j2 * G + g2) * G;
                 const double *yy = ys + a2 * G4 + p2;
                 double acc = 0.0;
-                for (int gc = 0; gc < G; ++gc) acc = fma(Kr[gc], yy[gc * 4], acc);
-                ss[t2] = S.dx[j2] * 0.25 * acc;
+                if (PRE && t2 == tid) {
+#pragma unroll
+                    for (int gc = 0; gc < GP; ++gc) acc = fma(Kr[gc], yy[gc * 4], acc);
+                    ss[t2] = dxq * acc;
+                } else {
+                    const double *Kp = S.transfer + ((size_t)j2 * G + g2) * G;
+                    for (int gc = 0; gc < G; ++gc) acc = fma(Kp[gc], yy[gc * 4], acc);
+                    ss[t2] = S.dx[j2] * 0.25 * acc;
+                }
             }
         }
         __syncthreads();
@@ -242,9 +277,6 @@ __global__ void __launch_bounds__(ST_THREADS) st_iterate_kernel(const IterParams
             *reinterpret_cast<double2 *>(out) = make_double2(x[0], x[1]);
             *reinterpret_cast<double2 *>(out + 2) = make_double2(x[2], x[3]);
         }
-        // wz / phiz / ys / ss are rewritten only after the next iteration's first barrier sequence; wz is written
-        // before that barrier by threads that may still be read by slower ones here -> one more barrier
-        __syncthreads();
     }
     rmax = warp_max(rmax);
     if (lane == 0) atomicMax(P.resid_inf, resid_bits(rmax));
@@ -264,16 +296,20 @@ int launch_st_factor(oci_ctx *ctx)
     if (!st_supported(ctx)) return OCI_E_UNSUPPORTED;
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream));
-    const size_t total = (size_t)ctx->J * ctx->G;
+    const size_t total = (size_t)ctx->J * ctx->G * ctx->N;
     size_t g1 = (total + 127) / 128;
-    if (g1 > (size_t)ctx->num_sms * 16) g1 = (size_t)ctx->num_sms * 16;
-    st_setup_kernel<<<(int)g1, 128, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg);
+    if (g1 > (size_t)ctx->num_sms * 32) g1 = (size_t)ctx->num_sms * 32;
+    st_setup_kernel<<<(int)g1, 128, 0, ctx->stream>>>(P, ctx->st_LinvT);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    size_t g3 = ((size_t)ctx->J * ctx->G * 16 + 255) / 256;
+    if (g3 > (size_t)ctx->num_sms * 16) g3 = (size_t)ctx->num_sms * 16;
+    st_wsum_kernel<<<(int)g3, 256, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
     size_t g2 = ((size_t)ctx->J + CAP_WARPS - 1) / CAP_WARPS;
     if (g2 > (size_t)ctx->num_sms * 4) g2 = (size_t)ctx->num_sms * 4;
     st_cap_kernel<<<(int)g2, CAP_WARPS * 32, 0, ctx->stream>>>(P, ctx->st_Wg, ctx->st_Cinv, ctx->info);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
-    return 2;
+    return 3;
 }
 
 int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
@@ -282,10 +318,20 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
     S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
     const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
     const size_t smem = sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 + (size_t)3 * CPB * G4);
-    int grid = (ctx->J + CPB - 1) / CPB;
-    if (grid > ctx->num_sms * 8) grid = ctx->num_sms * 8;
-    if (want_l2) st_iterate_kernel<true><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);
-    else st_iterate_kernel<false><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);
+    const int grid = (ctx->J + CPB - 1) / CPB; // one batch of CPB cells per CTA: CTA turnover hides the load latency
+#define OCI_ST_LAUNCH(GC_)                                                                                         \
+    do {                                                                                                           \
+        if (want_l2) st_iterate_kernel<true, GC_><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);                  \
+        else st_iterate_kernel<false, GC_><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);                         \
+    } while (0)
+    switch (ctx->G) {
+    case 1: OCI_ST_LAUNCH(1); break;
+    case 2: OCI_ST_LAUNCH(2); break;
+    case 4: OCI_ST_LAUNCH(4); break;
+    case 8: OCI_ST_LAUNCH(8); break;
+    default: OCI_ST_LAUNCH(0); break;
+    }
+#undef OCI_ST_LAUNCH
     OCI_CUDA_TRY(ctx, cudaGetLastError());
     return 1;
 }
