@@ -85,7 +85,13 @@ int oci_last_cuda_error(const oci_ctx *ctx);
 
 /* Tuning knobs (all optional). Known keys: "iterate_kernel" (0 = plain one-CTA-per-cell, 1 = pipelined
  * bulk-copy streaming kernel [default]), "iterate_stages", "iterate_ctas_per_sm", "factor_kernel"
- * (0 = shared-memory elimination, 1 = auto), "use_graph", "refactor_every_step" (1 = oci_step / si_step redo
+ * (0 = shared-memory elimination, 1 = register-tiled kernels [default]: two warps per cell for n = 64, clusters of
+ * n/64 CTAs for n = 128, 192, 256; 2 = the cluster-capable kernel also for n = 64), "solve_mode" (0 = dense
+ * [default]: a2 eliminates the dense A_j with partial pivoting and a5 streams A_j^{-1}, the paper's method;
+ * 1 = structured: A_j = D - U V^T with D the 4x4 blocks of Eq. 8b and rank 4G (Eq. 10 / 40b), a2 inverts the
+ * blocks and the 4G x 4G capacitance matrix with partial pivoting, a5 applies them -- the same iteration to
+ * rounding, 4n + 16 G^2 doubles of factors per cell-solve instead of n^2; needs G <= 8; switching invalidates the
+ * factors), "use_graph", "refactor_every_step" (1 = oci_step / si_step redo
  * a1+a2 at the start of every step as Alg. 2 prints it; 0 [default] = only when dt changed), "si_lanes" (ordinates x
  * groups swept by one CTA of the SI sweep kernel: 4, 8 [default] or 16). Returns -2 for an unknown key. */
 int oci_set_option(oci_ctx *ctx, const char *key, int64_t value);
@@ -142,7 +148,8 @@ int oci_step_host(oci_ctx *ctx, int32_t scheme, const double *q_host, double tol
 
 /* Debug / parity helpers (tests only). A_host, Ainv_host: [n][n] row-major. [sync] */
 int oci_debug_get_matrix(oci_ctx *ctx, int32_t cell, double *A_host);   /* assembled, un-eliminated A_j  */
-int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host);/* what oci_factor stored for j   */
+int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host);/* what oci_factor stored for j
+                                                                          (OCI_E_UNSUPPORTED in solve_mode 1) */
 int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev);               /* [J][n] c_j of a3 [async]       */
 
 /* Device time (ms, CUDA events on the context's stream) of the most recent call of each kind:
