@@ -116,6 +116,7 @@ __global__ void si_source_kernel(StopCheck stop, ProblemView P, int lpc, const d
 constexpr int TC = 64;         // sweep steps per tile
 constexpr int SW_STAGES = 4;
 constexpr int SW_THREADS = 64;
+constexpr int SW_AHEAD = 4;    // cells of look-ahead of the chain warp's shared-memory loads
 
 template <int LPC>
 __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, int J, int N, int G, int bc_left,
@@ -191,32 +192,43 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
         mbar_wait(&full[st], (t / SW_STAGES) & 1);
         const int cells = min(TC, J - t * TC);
         if (active) {
+            // software-pipelined: the coefficients of cell u + SW_AHEAD are loaded from shared memory while cell u
+            // is on the chain, so that the two dependent DFMAs never wait for a shared-memory load
+            double2 t0[SW_AHEAD], t1[SW_AHEAD], bb[SW_AHEAD];
+#pragma unroll
+            for (int d = 0; d < SW_AHEAD; ++d) {
+                t0[d] = *reinterpret_cast<const double2 *>(&Ts[st][d][l][0]);
+                t1[d] = *reinterpret_cast<const double2 *>(&Ts[st][d][l][2]);
+                bb[d] = *reinterpret_cast<const double2 *>(&Bs[st][d][l][0]);
+            }
+#define OCI_SWEEP_CELL(GUARD)                                                                                      \
+    do {                                                                                                           \
+        if (!(GUARD) || u0 + d < cells) {                                                                          \
+            *reinterpret_cast<double2 *>(op) = make_double2(in0, in1);                                             \
+            op += ostep;                                                                                           \
+            const double o0 = fma(t0[d].x, in0, fma(t0[d].y, in1, bb[d].x));                                       \
+            const double o1 = fma(t1[d].x, in0, fma(t1[d].y, in1, bb[d].y));                                       \
+            in0 = o0;                                                                                              \
+            in1 = o1;                                                                                              \
+        }                                                                                                          \
+        const int un = min(u0 + d + SW_AHEAD, TC - 1); /* stays inside the stage; unused past `cells` */           \
+        t0[d] = *reinterpret_cast<const double2 *>(&Ts[st][un][l][0]);                                             \
+        t1[d] = *reinterpret_cast<const double2 *>(&Ts[st][un][l][2]);                                             \
+        bb[d] = *reinterpret_cast<const double2 *>(&Bs[st][un][l][0]);                                             \
+    } while (0)
             if (cells == TC) {
-#pragma unroll 16
-                for (int u = 0; u < TC; ++u) {
-                    const double2 t0 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][0]);
-                    const double2 t1 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][2]);
-                    const double2 bb = *reinterpret_cast<const double2 *>(&Bs[st][u][l][0]);
-                    *reinterpret_cast<double2 *>(op) = make_double2(in0, in1);
-                    op += ostep;
-                    const double o0 = fma(t0.x, in0, fma(t0.y, in1, bb.x));
-                    const double o1 = fma(t1.x, in0, fma(t1.y, in1, bb.y));
-                    in0 = o0;
-                    in1 = o1;
+#pragma unroll 4
+                for (int u0 = 0; u0 < TC; u0 += SW_AHEAD) {
+#pragma unroll
+                    for (int d = 0; d < SW_AHEAD; ++d) OCI_SWEEP_CELL(false);
                 }
             } else {
-                for (int u = 0; u < cells; ++u) {
-                    const double2 t0 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][0]);
-                    const double2 t1 = *reinterpret_cast<const double2 *>(&Ts[st][u][l][2]);
-                    const double2 bb = *reinterpret_cast<const double2 *>(&Bs[st][u][l][0]);
-                    *reinterpret_cast<double2 *>(op) = make_double2(in0, in1);
-                    op += ostep;
-                    const double o0 = fma(t0.x, in0, fma(t0.y, in1, bb.x));
-                    const double o1 = fma(t1.x, in0, fma(t1.y, in1, bb.y));
-                    in0 = o0;
-                    in1 = o1;
+                for (int u0 = 0; u0 < cells; u0 += SW_AHEAD) {
+#pragma unroll
+                    for (int d = 0; d < SW_AHEAD; ++d) OCI_SWEEP_CELL(true);
                 }
             }
+#undef OCI_SWEEP_CELL
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
