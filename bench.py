@@ -78,6 +78,23 @@ def algorithmic_bytes_per_cell_solve(n: int, G: int) -> int:
     return 8 * n * n + 24 * n + 64 * G
 
 
+def max_over_ranks(value: float, device="cuda") -> float:
+    """Timing contract: the slowest rank's time. No-op without an initialised process group (N = 1)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, J: int, iterations_per_rank: int, ms: float) -> float:
+    """Replicas only: every rank solves the same problem, so the job did world x J x iterations
+    cell-solves in the slowest rank's time."""
+    return world * J * iterations_per_rank / (ms * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
 
@@ -236,12 +253,8 @@ def run_ours(args):
             kernel_ms_total += kms
         ev1.record()
         barrier()
-    ms_total = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * J * iters_total / (ms_total * 1e-3)
+    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    value = whole_job_value(world, J, iters_total, ms_total)
 
     # ---- structured cell solve, same sequence, reported beside (not part of `value`) -----------
     st = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}", options={"solve_mode": 1})
@@ -263,11 +276,7 @@ def run_ours(args):
         st_factor_ms.append(st.last_timing(0)[0])
     ev1.record()
     barrier()
-    st_ms_total = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([st_ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        st_ms_total = float(t.item())
+    st_ms_total = max_over_ranks(ev0.elapsed_time(ev1))
     st_diff = float((oci.scalar_flux() - st.scalar_flux()).abs().max().item())
 
     # ---- SI comparator, same sequence (reported beside, not part of `value`) ----------------------------------
@@ -298,12 +307,8 @@ def run_ours(args):
         it, _, _ = e2e.step_host(0, q_host, phi_host, tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
         e2e_iters += it
     barrier()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_value = world * J * e2e_iters / e2e_s
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e_value = whole_job_value(world, J, e2e_iters, e2e_s * 1e3)
     nbytes = J * G * 4 * 8
 
     if rank != 0:
@@ -331,7 +336,7 @@ def run_ours(args):
     st_achieved = st_bytes / (st_launch_ms * 1e-3) / 1e9
     structured = {
         "what": "SURVEY 8(f) row f1: structured cell solve A_j = D - U V^T (solve_mode = 1), same steps, same stop rule",
-        "value": world * J * st_iters / (st_ms_total * 1e-3), "unit": UNIT, "ms_per_step": st_ms_total / K,
+        "value": whole_job_value(world, J, st_iters, st_ms_total), "unit": UNIT, "ms_per_step": st_ms_total / K,
         "iterations_total": st_iters, "factor_ms": statistics.mean(st_factor_ms),
         "max_abs_phi_minus_dense_path": st_diff,
         "roofline": {"bound": "hbm", "kernel": "st_iterate_kernel", "achieved": st_achieved, "peak": peak, "unit": "GB/s",
