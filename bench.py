@@ -47,10 +47,12 @@ MAX_ITERS = 4000
 METRIC = "oci_cell_solves_per_s"
 UNIT = "cell-solves/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of one oci_iterate_wpc_kernel<2,0> launch on this workload, from the
-# `ncu --set full` capture summarised in profiles/r01_c_ncu_full.md (2.214780 GB read + 37.87 MB written).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 2252651360
-# same for one factor launch (factor_w2_kernel): 8.8 MB read + 2.097 GB written
-NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2105848448
+# `ncu --set full` capture summarised in profiles/r01_c_ncu_full.md (2.214779 GB read + 38.01 MB written).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 2252789624
+# same for one factor launch (factor_w2_kernel): 2.07 MB read + 2.097311 GB written
+NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2099381528
+# same for one st_iterate_kernel<0,1> launch: 212.89 MB read + 25.13 MB written
+NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH = 238012160
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
                                                     # .sum.peak_sustained = 64 per SM) x 2 flop x clocks.max.sm
 
@@ -340,7 +342,7 @@ def run_ours(args):
         "iterations_total": st_iters, "factor_ms": statistics.mean(st_factor_ms),
         "max_abs_phi_minus_dense_path": st_diff,
         "roofline": {"bound": "hbm", "kernel": "st_iterate_kernel", "achieved": st_achieved, "peak": peak, "unit": "GB/s",
-                     "frac": st_achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": st_achieved / peak, "traffic": NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": st_bytes, "avg_launch_ms": st_launch_ms,
                      "kernel_share_of_step": st_kernel_ms / st_ms_total},
     }
