@@ -166,16 +166,15 @@ __device__ __forceinline__ double rcp_nr(double x)
 
 // Phase P of the blocked Gauss-Jordan (both register-tiled kernels): one warp eliminates its n x 8 panel `a`
 // (lane l holds the rows {64 s + 2 l, 64 s + 2 l + 1}, s < TR / 2, register row rr = 2 s + e) with warp-level
-// operations only. usedmask: bit rr set = that row of this lane was a pivot row of an earlier step. bc: 20 doubles of
-// shared memory private to the warp. Returns the pivot rows in Rl and whether a zero / non-finite pivot was met.
+// operations only. usedmask: bit rr set = that row of this lane was a pivot row of an earlier step. Returns the pivot
+// rows in Rl and whether a zero / non-finite pivot was met.
 template <int TR>
-__device__ __forceinline__ bool panel_eliminate(double (&a)[TR][8], unsigned usedmask, double *bc, int lane,
-                                                int (&Rl)[FR_NB])
+__device__ __forceinline__ bool panel_eliminate(double (&a)[TR][8], unsigned usedmask, int lane, int (&Rl)[FR_NB])
 {
     constexpr unsigned FULL = 0xffffffffu;
     // Everything that does not depend on WHICH row wins (1/candidate, the candidate row scaled by it)
     // is computed by every lane for its own candidate in the shadow of the arg-max reduction; the
-    // winner then only has to publish 64 bytes.
+    // winner's scaled row is then broadcast by shuffles.
     bool bad = false;
     unsigned um = usedmask;
 #pragma unroll
@@ -224,21 +223,12 @@ __device__ __forceinline__ bool panel_eliminate(double (&a)[TR][8], unsigned use
                          (TR - 1); // warp-uniform
         Rl[b] = 64 * (rr_r >> 1) + 2 * src + (rr_r & 1);
         const bool mine = lane == src;
-        // pivot row (already scaled) through a per-warp shared-memory slot (two slots alternate)
-        double *slot = bc + (b & 1) * 10;
-        if (mine) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-                reinterpret_cast<double2 *>(slot)[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
-        }
-        __syncwarp();
+        // pivot row (already scaled): broadcast from the winner's registers by shuffles -- no shared-memory round trip
+        // and no memory barrier in the instruction stream, so the trailing updates of this step can overlap the
+        // next step's arg-max
         double sp[8];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const double2 t = reinterpret_cast<const double2 *>(slot)[c];
-            sp[2 * c] = t.x;
-            sp[2 * c + 1] = t.y;
-        }
+        for (int c = 0; c < 8; ++c) sp[c] = __shfl_sync(FULL, scl[c], src);
 #pragma unroll
         for (int rr = 0; rr < TR; ++rr) {
             const bool is_p = mine && rr == rr_r;
@@ -262,7 +252,6 @@ __device__ __forceinline__ bool panel_eliminate(double (&a)[TR][8], unsigned use
 template <int NQ> struct FrShared {
     double Z[2][FR_NB][64 * NQ];          // [buf][b][row]
     double Rrow[2][FR_NB][64];            // [buf][b][local column]
-    double bcast[FR_THREADS / 32][2][10]; // per warp: pivot row (8) + 1/pivot of a panel step, two slots
     int R[2][FR_NB];                      // pivot rows of the panel
     int sing[2];                          // panel met a zero / non-finite pivot
     int rho[64 * NQ], rhoinv[64 * NQ];
@@ -279,7 +268,6 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int n_clusters = gridDim.x / NQ, cluster_id = blockIdx.x / NQ;
     const int N = P.N, G = P.G;
-    const unsigned FULL = 0xffffffffu;
     unsigned gp = 0; // running panel counter: selects the shared-memory buffer
 
     auto cluster_barrier = [&]() {
@@ -344,7 +332,7 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
             if (owner) {
                 // ================= phase P: eliminate the n x 8 panel inside this warp =====================
                 int Rl[FR_NB];
-                const bool bad = panel_eliminate<TR>(a, usedmask, &sh.bcast[w][0][0], lane, Rl);
+                const bool bad = panel_eliminate<TR>(a, usedmask, lane, Rl);
                 // ---- publish Z = T[:, R] - I[:, R], R and the singular flag to every CTA of the cluster
 #pragma unroll
                 for (int t = 0; t < NQ; ++t) {
@@ -446,7 +434,6 @@ constexpr int W2_THREADS = 64;
 struct W2Shared {
     double S[2][32][64];           // [warp][local column][row]: shadow copy of the warp's tile, refreshed every panel
     double Z[2][FR_NB][64];        // [buf][b][row]
-    double bcast[2][20];
     int R[2][FR_NB];
     int sing[2];
     int rho[64], rhoinv[64];
@@ -519,7 +506,7 @@ __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restr
                             for (int c = 0; c < 8; ++c) t[e][c] = a[8 * k + c][e];
                     }
                 int Rl[FR_NB];
-                const bool bad = panel_eliminate<2>(t, usedmask, &sh.bcast[w][0], lane, Rl);
+                const bool bad = panel_eliminate<2>(t, usedmask, lane, Rl);
 #pragma unroll
                 for (int b = 0; b < FR_NB; ++b) {
                     double2 z;
