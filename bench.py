@@ -341,7 +341,7 @@ def run_ours(args):
         "value": whole_job_value(world, J, st_iters, st_ms_total), "unit": UNIT, "ms_per_step": st_ms_total / K,
         "iterations_total": st_iters, "factor_ms": statistics.mean(st_factor_ms),
         "max_abs_phi_minus_dense_path": st_diff,
-        "roofline": {"bound": "hbm", "kernel": "st_iterate_kernel", "achieved": st_achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": "st_iterate_pipe_kernel<0,1>", "achieved": st_achieved, "peak": peak, "unit": "GB/s",
                      "frac": st_achieved / peak, "traffic": NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": st_bytes, "avg_launch_ms": st_launch_ms,
                      "kernel_share_of_step": st_kernel_ms / st_ms_total},

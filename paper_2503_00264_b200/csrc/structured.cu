@@ -297,6 +297,262 @@ __global__ void __launch_bounds__(ST_THREADS, ST_MINB) st_iterate_kernel(const I
     }
 }
 
+// ============================================================================================================
+// Persistent, bulk-copy-pipelined version of st_iterate_kernel (the production kernel of solve_mode 1).
+// ============================================================================================================
+// Same arithmetic, thread for thread. One CTA per SM owns a contiguous range of cells and walks it in batches of
+// CPB = 256 / (G N) cells; per batch one producer thread issues four 1-D bulk async copies (the batch's 4x4 block
+// inverses, c_j, Psi^(l) of the batch and its two neighbour cells, C^-1 -- each contiguous in HBM by construction of
+// the layouts) into a ring of `stages` shared-memory stages guarded by mbarriers, so that HBM stays busy while the
+// 256 consumer threads work out of shared memory. The blocks are re-read from shared memory for x = z + D^-1 U y
+// instead of being held in registers across the barriers.
+constexpr int STP_CONSUMERS = ST_THREADS;
+constexpr int STP_THREADS = ST_THREADS + 32;
+constexpr int STP_MAX_STAGES = 6;
+
+struct StStage {                // element offsets inside one stage (all multiples of 2 doubles)
+    int Lt, cs, nb, Ci, doubles;
+};
+
+__host__ __device__ inline StStage st_stage_layout(int N, int G)
+{
+    const int GN = G * N, n = 4 * GN, G4 = 4 * G, CPB = ST_THREADS / GN;
+    StStage s;
+    s.Lt = 0;
+    s.cs = s.Lt + CPB * 16 * GN;
+    s.nb = s.cs + CPB * n;
+    s.Ci = s.nb + (CPB + 2) * n;
+    s.doubles = (s.Ci + CPB * G4 * G4 + 15) & ~15; // stages stay 128-byte aligned
+    return s;
+}
+
+template <bool WANT_L2, int GC>
+__global__ void __launch_bounds__(STP_THREADS, 2) st_iterate_pipe_kernel(const IterParams P, const StParams S, int stages)
+{
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
+    extern __shared__ __align__(128) unsigned char stp_smem[];
+    const int N = P.N, G = GC > 0 ? GC : P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
+    const int CPB = ST_THREADS / GN;
+    const StStage lay = st_stage_layout(N, G);
+    uint64_t *full = reinterpret_cast<uint64_t *>(stp_smem);
+    uint64_t *empty = full + STP_MAX_STAGES;
+    double *mu_s = reinterpret_cast<double *>(empty + STP_MAX_STAGES); // [N]
+    double *w_s = mu_s + N;                                           // [N]
+    double *wz = w_s + N;                                             // [CPB][GN][4]
+    double *phiz = wz + (size_t)CPB * GN * 4;                         // [CPB][4G]
+    double *ys = phiz + (size_t)CPB * G4;                             // [CPB][4G]
+    double *ss = ys + (size_t)CPB * G4;                               // [CPB][4G]
+    size_t off = (size_t)((unsigned char *)(ss + (size_t)CPB * G4) - stp_smem);
+    off = (off + 127) & ~(size_t)127;
+    double *ring = reinterpret_cast<double *>(stp_smem + off);        // stages x lay.doubles
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        for (int s = 0; s < stages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], STP_CONSUMERS / 32); }
+        fence_mbar_init();
+    }
+    for (int i = tid; i < N; i += STP_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    __syncthreads();
+
+    const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
+    const int cell1 = (int)(((long long)J * (blockIdx.x + 1)) / gridDim.x);
+
+    if (warp == STP_CONSUMERS / 32) {
+        // ===================== producer =====================================================================
+        if (lane == 0) {
+            int st = 0;
+            uint32_t ph = 0;
+            for (int gb = cell0; gb < cell1; gb += CPB) {
+                const int nb = min(CPB, cell1 - gb);
+                mbar_wait(&empty[st], ph ^ 1);
+                double *base = ring + (size_t)st * lay.doubles;
+                const int lo = max(gb - 1, 0), hi = min(gb + nb, J - 1);
+                const uint32_t bL = (uint32_t)((size_t)nb * 16 * GN * sizeof(double));
+                const uint32_t bc = (uint32_t)((size_t)nb * n * sizeof(double));
+                const uint32_t bn = (uint32_t)((size_t)(hi - lo + 1) * n * sizeof(double));
+                const uint32_t bC = (uint32_t)((size_t)nb * G4 * G4 * sizeof(double));
+                mbar_arrive_expect_tx(&full[st], bL + bc + bn + bC);
+                bulk_g2s(base + lay.Lt, S.LinvT + (size_t)gb * 16 * GN, bL, &full[st]);
+                bulk_g2s(base + lay.cs, P.c + (size_t)gb * n, bc, &full[st]);
+                bulk_g2s(base + lay.nb + (size_t)(lo - (gb - 1)) * n, P.psi_old + (size_t)lo * n, bn, &full[st]);
+                bulk_g2s(base + lay.Ci, S.Cinv + (size_t)gb * G4 * G4, bC, &full[st]);
+                if (++st == stages) { st = 0; ph ^= 1; }
+            }
+        }
+        return;
+    }
+
+    // ========================= consumers ====================================================================
+    const int a = tid / GN, gm = tid - a * GN, g = gm / N, m = gm - g * N;
+    const bool lane_on = tid < CPB * GN;
+    const int rows = CPB * G4;
+    double rmax = 0.0, l2 = 0.0;
+    auto consumer_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(STP_CONSUMERS) : "memory"); };
+    auto small_sync = [&]() {
+        if (GC > 0) __syncwarp();
+        else consumer_sync();
+    };
+    // butterfly reduction over the ordinates: N a power of two <= 32 (groups of N lanes never straddle a warp then)
+    const bool shfl_reduce = N <= 32 && (N & (N - 1)) == 0;
+    double Kr_n[GC > 0 ? GC : 1], dxq_n = 0.0, phi_old_n = 0.0;
+    auto load_role2 = [&](int gb_, int nb_) {
+        if (GC > 0 && tid < rows && tid / G4 < nb_) {
+            const int a2 = tid / G4, r2 = tid - a2 * G4, j2 = gb_ + a2;
+            const double *Kp = S.transfer + ((size_t)j2 * G + (r2 >> 2)) * G;
+#pragma unroll
+            for (int gc = 0; gc < (GC > 0 ? GC : 1); ++gc) Kr_n[gc] = Kp[gc];
+            dxq_n = S.dx[j2]; // used (x 0.25) one batch later: nothing here waits for the load
+            phi_old_n = P.phi[(size_t)j2 * G4 + r2];
+        }
+    };
+    load_role2(cell0, min(CPB, cell1 - cell0));
+    int st = 0;
+    uint32_t ph = 0;
+    for (int gb = cell0; gb < cell1; gb += CPB) {
+        const int nb = min(CPB, cell1 - gb);
+        const double *base = ring + (size_t)st * lay.doubles;
+        const int j = gb + a;
+        const bool on = lane_on && a < nb;
+        // role-2 data that is not worth a bulk copy (this thread's row of K, dx, phi^(l)): plain loads, issued one
+        // batch ahead so that their latency never sits between two barriers
+        double Kr[GC > 0 ? GC : 1], dxq = dxq_n, phi_old = phi_old_n;
+#pragma unroll
+        for (int gc = 0; gc < (GC > 0 ? GC : 1); ++gc) Kr[gc] = Kr_n[gc];
+        load_role2(gb + CPB, min(CPB, cell1 - gb - CPB));
+        mbar_wait(&full[st], ph);
+        double z[4];
+        const double *Lp = base + lay.Lt + (size_t)a * 16 * GN + gm;
+        if (on) {
+            const double2 *cp = reinterpret_cast<const double2 *>(base + lay.cs + (size_t)a * n + gm * 4);
+            const double2 c01 = cp[0], c23 = cp[1];
+            double b[4] = {c01.x, c01.y, c23.x, c23.y};
+            const double mu = mu_s[m];
+            const double *self = base + lay.nb + (size_t)(a + 1) * n;
+            double v0 = 0.0, v1 = 0.0;
+            // a4: incident edge fluxes from Psi^(l) (Eq. 9c-d; closures Eq. 5a-b)
+            if (mu > 0.0) {
+                if (j > 0) { // 16-byte loads: two-way instead of eight-way bank conflicts at the 32-byte thread stride
+                    const double2 *up = reinterpret_cast<const double2 *>(self - n + gm * 4);
+                    v0 = up[0].y; v1 = up[1].y;
+                }
+                else if (P.bc_left == OCI_BC_REFLECTIVE) {
+                    v0 = self[(g * N + (N - 1 - m)) * 4 + 0]; v1 = self[(g * N + (N - 1 - m)) * 4 + 2];
+                } else if (P.bc_left == OCI_BC_PRESCRIBED) { v0 = P.inc_left[gm * 2]; v1 = P.inc_left[gm * 2 + 1]; }
+                b[0] = fma(mu, v0, b[0]);
+                b[2] = fma(mu, v1, b[2]);
+            } else {
+                if (j < J - 1) {
+                    const double2 *up = reinterpret_cast<const double2 *>(self + n + gm * 4);
+                    v0 = up[0].x; v1 = up[1].x;
+                }
+                else if (P.bc_right == OCI_BC_REFLECTIVE) {
+                    v0 = self[(g * N + (N - 1 - m)) * 4 + 1]; v1 = self[(g * N + (N - 1 - m)) * 4 + 3];
+                } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = P.inc_right[gm * 2]; v1 = P.inc_right[gm * 2 + 1]; }
+                b[1] = fma(-mu, v0, b[1]);
+                b[3] = fma(-mu, v1, b[3]);
+            }
+#pragma unroll
+            for (int p = 0; p < 4; ++p) // z = D^-1 b
+                z[p] = fma(Lp[(p * 4 + 3) * GN], b[3],
+                           fma(Lp[(p * 4 + 2) * GN], b[2], fma(Lp[(p * 4 + 1) * GN], b[1], Lp[(p * 4) * GN] * b[0])));
+        }
+        // phi_z = V^T z: the N ordinates of a (cell, group) are N consecutive lanes -> butterfly when N is a power of two
+        {
+            const double wm = on ? w_s[m] : 0.0;
+            double q[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) q[p] = on ? wm * z[p] : 0.0;
+            if (shfl_reduce) {
+                for (int o = N >> 1; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) q[p] += __shfl_xor_sync(0xffffffffu, q[p], o);
+                }
+                if (on && m == 0) {
+                    double2 *dst = reinterpret_cast<double2 *>(phiz + a * G4 + g * 4);
+                    dst[0] = make_double2(q[0], q[1]);
+                    dst[1] = make_double2(q[2], q[3]);
+                }
+            } else if (on) {
+                double2 *dst = reinterpret_cast<double2 *>(wz + (size_t)tid * 4);
+                dst[0] = make_double2(q[0], q[1]);
+                dst[1] = make_double2(q[2], q[3]);
+            }
+        }
+        consumer_sync();
+        for (int t2 = tid; !shfl_reduce && t2 < rows; t2 += STP_CONSUMERS) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4;
+            if (a2 < nb) {
+                const int g2 = r2 >> 2, p2 = r2 & 3;
+                const double *src = wz + ((size_t)a2 * GN + g2 * N) * 4 + p2;
+                double acc = 0.0;
+                for (int mm = 0; mm < N; ++mm) acc += src[mm * 4];
+                phiz[t2] = acc;
+            }
+        }
+        if (!shfl_reduce) small_sync();
+        for (int t2 = tid; t2 < rows; t2 += STP_CONSUMERS) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = gb + a2;
+            if (a2 < nb) {
+                const double *Cp = base + lay.Ci + (size_t)a2 * G4 * G4 + r2;
+                const double *pz = phiz + a2 * G4;
+                double y = 0.0;
+                for (int cc = 0; cc < G4; ++cc) y = fma(Cp[cc * G4], pz[cc], y);
+                const double po = (GC > 0 && t2 == tid) ? phi_old : P.phi[(size_t)j2 * G4 + r2];
+                ys[t2] = y;
+                P.phi[(size_t)j2 * G4 + r2] = y;
+                const double d = fabs(y - po);
+                rmax = (d > rmax || !(d == d)) ? d : rmax;
+            }
+        }
+        small_sync();
+        for (int t2 = tid; t2 < rows; t2 += STP_CONSUMERS) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = gb + a2;
+            if (a2 < nb) {
+                const int g2 = r2 >> 2, p2 = r2 & 3;
+                const double *yy = ys + a2 * G4 + p2;
+                double acc = 0.0;
+                if (GC > 0 && t2 == tid) {
+#pragma unroll
+                    for (int gc = 0; gc < (GC > 0 ? GC : 1); ++gc) acc = fma(Kr[gc], yy[gc * 4], acc);
+                    ss[t2] = dxq * 0.25 * acc;
+                } else {
+                    const double *Kp = S.transfer + ((size_t)j2 * G + g2) * G;
+                    for (int gc = 0; gc < G; ++gc) acc = fma(Kp[gc], yy[gc * 4], acc);
+                    ss[t2] = S.dx[j2] * 0.25 * acc;
+                }
+            }
+        }
+        consumer_sync();
+        if (on) { // x = z + D^-1 U y
+            const double *sv = ss + a * G4 + g * 4;
+            const double s0 = sv[0], s1 = sv[1], s2 = sv[2], s3 = sv[3];
+            double x[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p)
+                x[p] = fma(Lp[(p * 4 + 3) * GN], s3,
+                           fma(Lp[(p * 4 + 2) * GN], s2, fma(Lp[(p * 4 + 1) * GN], s1, fma(Lp[(p * 4) * GN], s0, z[p]))));
+            if (WANT_L2) {
+                const double *old = base + lay.nb + (size_t)(a + 1) * n + gm * 4;
+#pragma unroll
+                for (int p = 0; p < 4; ++p) { const double d = x[p] - old[p]; l2 = fma(d, d, l2); }
+            }
+            double *out = P.psi_new + (size_t)j * n + gm * 4;
+            *reinterpret_cast<double2 *>(out) = make_double2(x[0], x[1]);
+            *reinterpret_cast<double2 *>(out + 2) = make_double2(x[2], x[3]);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]); // this warp is done with the stage
+        if (++st == stages) { st = 0; ph ^= 1; }
+    }
+    rmax = warp_max(rmax);
+    if (lane == 0 && cell1 > cell0) atomicMax(P.resid_inf, resid_bits(rmax));
+    if (WANT_L2) {
+        l2 = warp_sum(l2);
+        if (lane == 0 && cell1 > cell0) atomicAdd(P.resid_l2, l2);
+    }
+}
+
 } // namespace
 
 bool st_supported(const oci_ctx *ctx) { return 4 * ctx->G <= 32 && ctx->G * ctx->N <= ST_THREADS; }
@@ -328,6 +584,54 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
     StParams S;
     S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
     const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
+    if (ctx->opt_iterate_kernel == 1) { // persistent bulk-copy pipeline; falls through when the ring would not fit
+        const StStage lay = st_stage_layout(ctx->N, ctx->G);
+        const size_t fixed = (size_t)2 * STP_MAX_STAGES * 8 + sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 +
+                                                                               (size_t)3 * CPB * G4) + 256;
+        // two CTAs per SM by default: each is a lock-step sequence of short latency-bound phases, two of them overlap
+        int ctas = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : 2;
+        if (ctas > 2) ctas = 2;
+        int stages = 0;
+        for (; ctas >= 1; --ctas) {
+            const size_t budget = ((size_t)ctx->max_smem_optin + 1024) / ctas - 1024; // 228 KB per SM, 1 KB reserved per CTA
+            stages = budget > fixed ? (int)((budget - fixed) / ((size_t)lay.doubles * 8)) : 0;
+            if (stages >= 2) break;
+        }
+        if (ctas < 1) ctas = 1;
+        if (stages > STP_MAX_STAGES) stages = STP_MAX_STAGES;
+        if (ctx->opt_stages > 0 && ctx->opt_stages < stages) stages = ctx->opt_stages;
+        if (stages >= 2) {
+            const size_t smem = fixed + (size_t)stages * lay.doubles * 8;
+            int grid = ctx->num_sms * ctas;
+            if (grid > (ctx->J + CPB - 1) / CPB) grid = (ctx->J + CPB - 1) / CPB;
+#define OCI_STP_LAUNCH(L2_, GC_)                                                                                   \
+    do {                                                                                                           \
+        static size_t attr = 0;                                                                                    \
+        if (attr < smem) {                                                                                         \
+            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(st_iterate_pipe_kernel<L2_, GC_>,                               \
+                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+            attr = smem;                                                                                           \
+        }                                                                                                          \
+        st_iterate_pipe_kernel<L2_, GC_><<<grid, STP_THREADS, smem, ctx->stream>>>(P, S, stages);                  \
+    } while (0)
+#define OCI_STP_G(GC_)                                                                                             \
+    do {                                                                                                           \
+        if (want_l2) OCI_STP_LAUNCH(true, GC_);                                                                    \
+        else OCI_STP_LAUNCH(false, GC_);                                                                           \
+    } while (0)
+            switch (ctx->G) {
+            case 1: OCI_STP_G(1); break;
+            case 2: OCI_STP_G(2); break;
+            case 4: OCI_STP_G(4); break;
+            case 8: OCI_STP_G(8); break;
+            default: OCI_STP_G(0); break;
+            }
+#undef OCI_STP_G
+#undef OCI_STP_LAUNCH
+            OCI_CUDA_TRY(ctx, cudaGetLastError());
+            return 1;
+        }
+    }
     const size_t smem = sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 + (size_t)3 * CPB * G4);
     const int grid = (ctx->J + CPB - 1) / CPB; // one batch of CPB cells per CTA: CTA turnover hides the load latency
 #define OCI_ST_LAUNCH(GC_)                                                                                         \

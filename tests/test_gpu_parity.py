@@ -310,10 +310,11 @@ def test_factor_kernels_agree_n64():
 ST = {"solve_mode": 1}
 
 
+@pytest.mark.parametrize("kernel", [1, 0])   # 1: persistent bulk-copy pipeline (default); 0: one batch of cells per CTA
 @pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
-def test_structured_per_iteration_parity(seed, J, N, G, bl, br):
+def test_structured_per_iteration_parity(seed, J, N, G, bl, br, kernel):
     p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
-    s, o = _solver(p, options=ST), _oracle(p)
+    s, o = _solver(p, options={"solve_mode": 1, "iterate_kernel": kernel}), _oracle(p)
     assert s.factor() == 0 and o.factor() == 0
     o.const_rhs()
     for l in range(6):
@@ -339,11 +340,12 @@ def test_structured_full_size_parity(name, make, n_it):
         assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
 
 
+@pytest.mark.parametrize("kernel", [1, 0])
 @pytest.mark.parametrize("rule", [0, 1])
 @pytest.mark.parametrize("k", [1, 5])
-def test_structured_step_loop_matches_oracle(rule, k):
+def test_structured_step_loop_matches_oracle(rule, k, kernel):
     p = W.random_problem(33, 61, 4, 2, bc_left=1, bc_right=2, dt=0.05)
-    s, o = _solver(p, options=ST), _oracle(p)
+    s, o = _solver(p, options={"solve_mode": 1, "iterate_kernel": kernel}), _oracle(p)
     for step in range(3):
         it_g, conv_g, _ = s.step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
         it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule)
