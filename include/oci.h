@@ -91,7 +91,7 @@ int oci_last_cuda_error(const oci_ctx *ctx);
  * 1 = structured: A_j = D - U V^T with D the 4x4 blocks of Eq. 8b and rank 4G (Eq. 10 / 40b), a2 inverts the
  * blocks and the 4G x 4G capacitance matrix with partial pivoting, a5 applies them -- the same iteration to
  * rounding, 4n + 16 G^2 doubles of factors per cell-solve instead of n^2; needs G <= 8; switching invalidates the
- * factors), "use_graph", "refactor_every_step" (1 = oci_step / si_step redo
+ * factors), "refactor_every_step" (1 = oci_step / si_step redo
  * a1+a2 at the start of every step as Alg. 2 prints it; 0 [default] = only when dt changed), "si_lanes" (ordinates x
  * groups swept by one CTA of the SI sweep kernel: 4, 8 [default] or 16). Returns -2 for an unknown key. */
 int oci_set_option(oci_ctx *ctx, const char *key, int64_t value);

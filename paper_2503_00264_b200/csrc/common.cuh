@@ -66,7 +66,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_use_graph, opt_refactor_every_step, opt_si_lanes, opt_solve_mode;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];

@@ -121,12 +121,6 @@ __global__ void __launch_bounds__(CAP_WARPS * 32) st_cap_kernel(ProblemView P, c
 // A CTA works on CPB = 256 / (G N) consecutive cells at a time. Loads are contiguous across the threads of a cell
 // (c_j and Psi: 32 bytes per thread; LinvT: ordinate-fastest; Cinv: column-major, one row per thread).
 constexpr int ST_THREADS = 256;
-#ifndef ST_RELOAD
-#define ST_RELOAD 0
-#endif
-#ifndef ST_MINB
-#define ST_MINB 3
-#endif
 
 struct StParams {
     const double *LinvT, *Cinv, *dx, *transfer;
@@ -136,7 +130,7 @@ struct StParams {
 // z and x need only __syncwarp, and for G <= 4 the thread's row of C^-1, its row of K and dx are loaded up front,
 // together with everything else, so that a CTA waits for HBM once); GC = 0: any G, CTA-wide barriers.
 template <bool WANT_L2, int GC>
-__global__ void __launch_bounds__(ST_THREADS, ST_MINB) st_iterate_kernel(const IterParams P, const StParams S)
+__global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterParams P, const StParams S)
 {
     if (stop_reached(P.stop)) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
@@ -271,11 +265,6 @@ __global__ void __launch_bounds__(ST_THREADS, ST_MINB) st_iterate_kernel(const I
             const double *sv = ss + a * G4 + g * 4;
             const double s0 = sv[0], s1 = sv[1], s2 = sv[2], s3 = sv[3];
             double x[4];
-            if (ST_RELOAD) { // the block is re-read (an L1 hit) instead of kept in 32 registers across the barriers
-                const double *Lp = S.LinvT + (size_t)j * 16 * GN + gm;
-#pragma unroll
-                for (int k = 0; k < 16; ++k) L[k] = __ldg(Lp + (size_t)k * GN);
-            }
 #pragma unroll
             for (int p = 0; p < 4; ++p)
                 x[p] = fma(L[p * 4 + 3], s3, fma(L[p * 4 + 2], s2, fma(L[p * 4 + 1], s1, fma(L[p * 4], s0, z[p]))));
