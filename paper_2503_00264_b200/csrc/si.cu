@@ -108,14 +108,15 @@ __global__ void si_source_kernel(StopCheck stop, ProblemView P, int lpc, const d
 
 // a10: the sweep. One CTA per group of LPC chains (ordinates (g,m)), warp-specialised:
 //   warp 1, one thread : issues one bulk async copy per tile (TC sweep steps x LPC chains) of the 2x2 maps and one of
-//                        the constant terms into a ring of SW_STAGES shared-memory stages (mbarrier handshake);
+//                        the constant terms into a ring of 3-4 shared-memory stages (mbarrier handshake);
 //   warp 0, lane = chain: runs the serial chain  in_{jj+1} = b_jj + T_jj in_jj  out of shared memory -- per cell three
-//                        conflict-free 16-byte loads, four DFMAs (two dependent), one 16-byte store of the incident
-//                        flux that si_finish needs. Nothing else is on the chain warp's instruction stream.
+//                        conflict-free 16-byte loads, four DFMAs (two dependent), one 16-byte shared-memory store of
+//                        the incident flux that si_finish needs. Nothing else is on its instruction stream.
+//   warp 2              : copies the finished tiles of incident fluxes from shared memory to in_out[j][gm][2].
 // The chain is the latency floor of a sweep "serial in space": J x 2 dependent DFMAs.
 constexpr int TC = 64;         // sweep steps per tile
-constexpr int SW_STAGES = 4;
-constexpr int SW_THREADS = 64;
+__host__ __device__ constexpr int sw_stages(int lpc) { return lpc >= 16 ? 3 : 4; } // ring depth (227 KB per CTA)
+constexpr int SW_THREADS = 96;
 constexpr int SW_AHEAD = 4;    // cells of look-ahead of the chain warp's shared-memory loads
 
 template <int LPC>
@@ -128,20 +129,23 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
                                                               const double *__restrict__ inc_right,
                                                               double *__restrict__ in_out)
 {
+    constexpr int NST = sw_stages(LPC);
     extern __shared__ __align__(128) unsigned char sw_smem[];
     typedef double (*TsT)[TC][LPC][4];
     typedef double (*BsT)[TC][LPC][2];
-    TsT Ts = reinterpret_cast<TsT>(sw_smem);                                              // [SW_STAGES][TC][LPC][4]
-    BsT Bs = reinterpret_cast<BsT>(sw_smem + sizeof(double) * SW_STAGES * TC * LPC * 4); // [SW_STAGES][TC][LPC][2]
-    uint64_t *full = reinterpret_cast<uint64_t *>(sw_smem + sizeof(double) * SW_STAGES * TC * LPC * 6);
-    uint64_t *empty = full + SW_STAGES;
+    TsT Ts = reinterpret_cast<TsT>(sw_smem);                                              // [NST][TC][LPC][4]
+    BsT Bs = reinterpret_cast<BsT>(sw_smem + sizeof(double) * NST * TC * LPC * 4); // [NST][TC][LPC][2]
+    BsT Os = reinterpret_cast<BsT>(sw_smem + sizeof(double) * NST * TC * LPC * 6); // incident fluxes found
+    uint64_t *full = reinterpret_cast<uint64_t *>(sw_smem + sizeof(double) * NST * TC * LPC * 8);
+    uint64_t *empty = full + NST;     // stage free again: chain warp done reading AND writer warp done copying
+    uint64_t *outfull = empty + NST;  // chain warp finished the tile: Os[stage] complete
     if (stop_reached(stop)) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int GN = G * N, n = 4 * GN;
     const int gm0 = blockIdx.x * LPC;
     const int n_tiles = (J + TC - 1) / TC;
     if (tid == 0) {
-        for (int s = 0; s < SW_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 2); mbar_init(&outfull[s], 1); }
         fence_mbar_init();
     }
     __syncthreads();
@@ -151,8 +155,8 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
             const double *Tsrc = T2sw + (size_t)blockIdx.x * J * LPC * 4;
             const double *Bsrc = bsw + (size_t)blockIdx.x * J * LPC * 2;
             for (int t = 0; t < n_tiles; ++t) {
-                const int st = t % SW_STAGES;
-                mbar_wait(&empty[st], ((t / SW_STAGES) & 1) ^ 1);
+                const int st = t % NST;
+                mbar_wait(&empty[st], ((t / NST) & 1) ^ 1);
                 const int cells = min(TC, J - t * TC);
                 const uint32_t bt = (uint32_t)(cells * LPC * 4 * sizeof(double));
                 const uint32_t bb = (uint32_t)(cells * LPC * 2 * sizeof(double));
@@ -160,6 +164,27 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
                 bulk_g2s(&Ts[st][0][0][0], Tsrc + (size_t)t * TC * LPC * 4, bt, &full[st]);
                 bulk_g2s(&Bs[st][0][0][0], Bsrc + (size_t)t * TC * LPC * 2, bb, &full[st]);
             }
+        }
+        return;
+    }
+    if (warp == 2) { // writer: Os[stage][u][l] -> in_out[cell of sweep step t TC + u][gm0 + l]
+        const int l = lane % LPC, u_first = lane / LPC, gmw = gm0 + l;
+        const bool on = gmw < GN;
+        const bool fwd_w = on ? mu[gmw % N] > 0.0 : true;
+        for (int t = 0; t < n_tiles; ++t) {
+            const int st = t % NST;
+            mbar_wait(&outfull[st], (t / NST) & 1);
+            const int cells = min(TC, J - t * TC);
+            if (on) {
+                for (int u = u_first; u < cells; u += 32 / LPC) {
+                    const size_t jj = (size_t)t * TC + u;
+                    const size_t j = fwd_w ? jj : (size_t)(J - 1) - jj;
+                    *reinterpret_cast<double2 *>(in_out + (j * GN + gmw) * 2) =
+                        *reinterpret_cast<const double2 *>(&Os[st][u][l][0]);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
         }
         return;
     }
@@ -182,14 +207,11 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
             in1 = ip[1];
         }
     }
-    // in_out[j][gm][2]: element stride between consecutive sweep steps of this chain
-    const long long ostep = fwd ? (long long)GN * 2 : -(long long)GN * 2;
-    double *op = in_out + ((fwd ? (size_t)0 : (size_t)(J - 1)) * GN + (active ? gm : 0)) * 2;
     const int l = active ? lane : 0;
 
     for (int t = 0; t < n_tiles; ++t) {
-        const int st = t % SW_STAGES;
-        mbar_wait(&full[st], (t / SW_STAGES) & 1);
+        const int st = t % NST;
+        mbar_wait(&full[st], (t / NST) & 1);
         const int cells = min(TC, J - t * TC);
         if (active) {
             // software-pipelined: the coefficients of cell u + SW_AHEAD are loaded from shared memory while cell u
@@ -204,8 +226,7 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
 #define OCI_SWEEP_CELL(GUARD)                                                                                      \
     do {                                                                                                           \
         if (!(GUARD) || u0 + d < cells) {                                                                          \
-            *reinterpret_cast<double2 *>(op) = make_double2(in0, in1);                                             \
-            op += ostep;                                                                                           \
+            *reinterpret_cast<double2 *>(&Os[st][u0 + d][l][0]) = make_double2(in0, in1);                          \
             const double o0 = fma(t0[d].x, in0, fma(t0[d].y, in1, bb[d].x));                                       \
             const double o1 = fma(t1[d].x, in0, fma(t1[d].y, in1, bb[d].y));                                       \
             in0 = o0;                                                                                              \
@@ -231,7 +252,7 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
 #undef OCI_SWEEP_CELL
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st]);
+        if (lane == 0) { mbar_arrive(&outfull[st]); mbar_arrive(&empty[st]); }
     }
 }
 
@@ -329,7 +350,7 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_pr
     const int sweep_grid = (GN + lpc - 1) / lpc;
 #define OCI_SWEEP(LPC_)                                                                                            \
     do {                                                                                                           \
-        const size_t smem = sizeof(double) * SW_STAGES * TC * LPC_ * 6 + 2 * SW_STAGES * sizeof(uint64_t);         \
+        const size_t smem = sizeof(double) * sw_stages(LPC_) * TC * LPC_ * 8 + 3 * sw_stages(LPC_) * sizeof(uint64_t);         \
         static bool attr_set = false;                                                                              \
         if (!attr_set) {                                                                                           \
             OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(si_sweep_kernel<LPC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
