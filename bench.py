@@ -396,6 +396,48 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------------------------
+# the paper's own timing experiment (Figs. 7-8) on this GPU. Not the headline.
+# ---------------------------------------------------------------------------------------------------------------
+def run_table2(args):
+    """Two-group problem of Table 2, L = 100 cm, vacuum, psi_0 = 0, first time step, delta =
+    Sigma_t,2 dx swept through dx, S16 and S32, dt = 10 s and 0.1 s. Like the paper, the time is that of the convergence
+    loop only (CUDA events around the iteration kernels; no assembly / elimination), stop rule = the paper's Eq. 12."""
+    import torch
+    from paper_2503_00264_b200 import OCISolver
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --table2 needs a CUDA device")
+    sig2, L, eps = 0.45468, 100.0, 1e-8
+    rows = []
+    for dt in (10.0, 0.1):
+        for N in (16, 32):
+            for delta in (10.0, 4.0, 1.0, 0.4, 0.1, 0.04, 0.01):
+                J = max(2, int(round(L * sig2 / delta)))
+                p = W.table2(J, N, dt, L)
+                row = {"dt": dt, "N": N, "n": p.n, "J": J, "delta": sig2 * L / J}
+                for name, scheme, opts in (("oci_dense", 0, {}), ("oci_structured", 0, {"solve_mode": 1}), ("si", 1, {})):
+                    best = None
+                    for rep in range(2):     # second repetition is warm
+                        s = OCISolver(p, options=opts)
+                        if scheme == 0:
+                            s.factor()
+                            it, conv, _ = s.step(tol=eps, max_iters=60000, check_every=16, stop_rule=1, advance=False)
+                            ms = s.last_timing(1)[0]
+                        else:
+                            it, conv, _ = s.si_step(tol=eps, max_iters=60000, check_every=16, stop_rule=1, advance=False)
+                            ms = s.last_timing(2)[0]
+                        best = ms if best is None else min(best, ms)
+                        del s
+                    row[name + "_iters"] = it
+                    row[name + "_converged"] = bool(conv)
+                    row[name + "_loop_ms"] = best
+                row["speedup_dense_over_si"] = row["si_loop_ms"] / row["oci_dense_loop_ms"]
+                row["speedup_structured_over_si"] = row["si_loop_ms"] / row["oci_structured_loop_ms"]
+                rows.append(row)
+    print(json.dumps({"experiment": "table2 delta sweep (PAPER.md:510-520, Figs. 7-8)", "unit": "ms per convergence loop",
+                      "stop_rule": "Eq. 12-13, eps = 1e-8", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -407,10 +449,14 @@ def main():
     ap.add_argument("--ref-cells", type=int, default=8192, help="cells per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-si", action="store_true", help="skip the SI comparator leg (profiling runs)")
+    ap.add_argument("--table2", action="store_true",
+                    help="instead of the headline benchmark: the paper's Table-2 delta sweep, OCI vs SI (SURVEY 8f row f3)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.impl == "reference":
+    if args.table2:
+        run_table2(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
