@@ -315,7 +315,7 @@ def run_ours(args):
 
     if rank != 0:
         return
-    # ---- roofline of the dominant kernel (oci_iterate_stream_kernel), from the timed region -----------------------
+    # ---- roofline of the dominant kernel (oci_iterate_wpc_kernel<2,0>), from the timed region -----------------------
     peak, peak_src = measured_peaks()
     launch_ms = kernel_ms_total / max(iters_total, 1)
     alg_bytes = algorithmic_bytes_per_cell_solve(n, G) * J

@@ -10,8 +10,9 @@
 //   r = max |phi^(l+1) - phi^(l)|    (and sum (Psi^(l+1)-Psi^(l))^2 for Eq. 12)
 // The kernel is HBM-bound: 8 n^2 bytes of A_j^{-1} per cell-solve against 2 n^2 flops. It therefore runs as
 // a persistent, warp-specialised streaming kernel: one producer thread per CTA issues 1-D bulk async copies
-// (cp.async.bulk, completion on mbarriers) into a multi-stage shared-memory ring; eight consumer warps
-// multiply the chunks as they land.
+// (cp.async.bulk, completion on mbarriers) into multi-stage shared-memory rings and the consumer warps multiply
+// the chunks as they land: oci_iterate_wpc_kernel (n = 64, 128, 256: a cell per consumer warp, the production
+// kernel of configs 3-5) and oci_iterate_stream_kernel (any other n: a team of threads per cell).
 #include "common.cuh"
 
 namespace {
