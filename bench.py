@@ -51,8 +51,8 @@ UNIT = "cell-solves/s"
 NCU_TRAFFIC_BYTES_PER_LAUNCH = 2252789624
 # same for one factor launch (factor_w2_kernel): 2.07 MB read + 2.097311 GB written
 NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2099381528
-# same for one st_iterate_kernel<0,1> launch: 212.89 MB read + 25.13 MB written
-NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH = 238012160
+# same for one st_iterate_pipe_kernel<0,1> launch (profiles/r01_d_ncu_full.md): 213.30 MB read + 21.86 MB written
+NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH = 235150848
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
                                                     # .sum.peak_sustained = 64 per SM) x 2 flop x clocks.max.sm
 
