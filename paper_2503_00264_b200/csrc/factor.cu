@@ -426,27 +426,37 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
 // panel phase is a serial, latency-bound instruction stream, so the throughput of the kernel is (cells in flight
 // per SM) / (length of that stream). Lane l of warp w holds the rows {2 l, 2 l + 1} of the columns
 // [32 w, 32 w + 32): 64 doubles per lane, 64 threads and ~17 KB of shared memory per cell, five cells per SM
-// (factor_reg_kernel<1>: three). Panel p (8 columns) belongs to warp p / 4, sub-tile p % 4 of its registers; the
-// owner copies that sub-tile out, eliminates it (panel_eliminate), publishes Z and R, and both warps apply the
-// rank-8 update to all their 32 columns (the owner then puts the eliminated sub-tile back over the result).
+// (factor_reg_kernel<1>: three). Panel p (8 columns) belongs to warp p / 4, sub-tile p % 4 of its registers. Every
+// panel, both warps refresh a shadow copy of their tiles in shared memory; the panel is then eliminated by BOTH warps
+// with one row per lane (read from the shadow): per pivot step a warp-level arg-max, the two candidates exchanged
+// through shared memory (one CTA barrier per step), an 8-wide row update -- about 70 instructions per step and no
+// idle warp, against 160 for one warp holding two rows per lane. Z goes to shared memory, the eliminated panel back
+// to its owner's registers, and both warps apply the rank-8 update to their 32 columns.
 constexpr int W2_THREADS = 64;
+
+struct W2Slot {                    // what a warp's local arg-max winner publishes in a pivot step
+    double row[FR_NB];             // its panel row, scaled by 1 / candidate (column b holds 1 / candidate)
+    unsigned long long key;        // bit pattern of |candidate| (0: this warp has no unused row)
+    int lane;
+    int pad;
+};
 
 struct W2Shared {
     double S[2][32][64];           // [warp][local column][row]: shadow copy of the warp's tile, refreshed every panel
-    double Z[2][FR_NB][64];        // [buf][b][row]
-    int R[2][FR_NB];
-    int sing[2];
+    double Z[FR_NB][64];           // [b][row]
+    double Pn[FR_NB][64];          // [c][row]: the eliminated panel on its way back to the owner's registers
+    W2Slot slot[2][2];             // [step parity][warp]
     int rho[64], rhoinv[64];
 };
 
 __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restrict__ Minv, int *info)
 {
     constexpr int n = 64, NPANEL = n / FR_NB;
+    constexpr unsigned FULL = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char w2_smem[];
     W2Shared &sh = *reinterpret_cast<W2Shared *>(w2_smem);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int N = P.N, G = P.G;
-    unsigned gp = 0;
 
     for (int cell = blockIdx.x; cell < P.J; cell += gridDim.x) {
         // ---- a1: assemble rows {2 lane, 2 lane + 1} x columns [32 w, 32 w + 32), bit-identical to a_entry().
@@ -487,73 +497,114 @@ __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restr
                 }
             }
         }
-        unsigned usedmask = 0;
+        bool used_r = false;   // row 32 w + lane (the row this lane holds during the panel phases) was a pivot row
         bool singular = false;
         double2 *Sw = reinterpret_cast<double2 *>(&sh.S[w][0][0]); // [local column][32 lanes] of double2
+        const int r = 32 * w + lane;
 
-        for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
-            const int buf = gp & 1;
-            const bool owner = (pnl >> 2) == w;
-            const int st = pnl & 3;
-            if (owner) {
-                double t[2][8];
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (k == st) {
-#pragma unroll
-                        for (int e = 0; e < 2; ++e)
-#pragma unroll
-                            for (int c = 0; c < 8; ++c) t[e][c] = a[8 * k + c][e];
-                    }
-                int Rl[FR_NB];
-                const bool bad = panel_eliminate<2>(t, usedmask, lane, Rl);
-#pragma unroll
-                for (int b = 0; b < FR_NB; ++b) {
-                    double2 z;
-                    z.x = t[0][b] - (Rl[b] == 2 * lane ? 1.0 : 0.0);
-                    z.y = t[1][b] - (Rl[b] == 2 * lane + 1 ? 1.0 : 0.0);
-                    *reinterpret_cast<double2 *>(&sh.Z[buf][b][2 * lane]) = z;
-                    if (lane == b) sh.R[buf][b] = Rl[b];
-                }
-                if (lane == 0) sh.sing[buf] = bad ? 1 : 0;
-                // the panel's own columns now hold T e_r; phase U must leave them alone (their shadow is zeroed below)
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (k == st) {
-#pragma unroll
-                        for (int e = 0; e < 2; ++e)
-#pragma unroll
-                            for (int c = 0; c < 8; ++c) a[8 * k + c][e] = t[e][c];
-                    }
-            }
-            // ---- shadow copy of this warp's tile (its OLD values are what phase U multiplies): conflict-free 16-byte stores
+        for (int pnl = 0; pnl < NPANEL; ++pnl) {
+            const int wo = pnl >> 2, st = pnl & 3;
+            const bool owner = wo == w;
+            // ---- shadow copy of this warp's tile: the panel phase reads the panel from it row by row, phase U its pivot
+            // rows (conflict-free 16-byte stores)
 #pragma unroll
             for (int c = 0; c < 32; ++c) Sw[c * 32 + lane] = make_double2(a[c][0], a[c][1]);
-            if (owner) {
-#pragma unroll
-                for (int c = 0; c < 8; ++c) Sw[(8 * st + c) * 32 + lane] = make_double2(0.0, 0.0);
-            }
-            __syncthreads(); // B1: Z, R, sing of this panel visible to both warps (and the shadow to this warp)
+            __syncthreads();
 
-            if (sh.sing[buf]) { singular = true; ++gp; break; }
-            int Rv[FR_NB];
-            {
-                const int4 r0 = *reinterpret_cast<const int4 *>(&sh.R[buf][0]);
-                const int4 r1 = *reinterpret_cast<const int4 *>(&sh.R[buf][4]);
-                Rv[0] = r0.x; Rv[1] = r0.y; Rv[2] = r0.z; Rv[3] = r0.w;
-                Rv[4] = r1.x; Rv[5] = r1.y; Rv[6] = r1.z; Rv[7] = r1.w;
-            }
+            // ================= phase P: both warps eliminate the 64 x 8 panel, ONE ROW PER LANE =================
+            double t[FR_NB];
+#pragma unroll
+            for (int c = 0; c < FR_NB; ++c) t[c] = sh.S[wo][8 * st + c][r];
+            int Rl[FR_NB];
+            bool bad = false;
 #pragma unroll
             for (int b = 0; b < FR_NB; ++b) {
-                if (lane == (Rv[b] >> 1)) usedmask |= 1u << (Rv[b] & 1);
-                if (w == 0 && lane == b) { sh.rho[FR_NB * pnl + b] = Rv[b]; sh.rhoinv[Rv[b]] = FR_NB * pnl + b; }
+                // local (warp) arg-max over the unused rows: first row of maximal |entry|
+                const unsigned long long key = used_r ? 0ull : (unsigned long long)__double_as_longlong(fabs(t[b]));
+                const unsigned khi = (unsigned)(key >> 32);
+                const unsigned mhi = __reduce_max_sync(FULL, khi);
+                // in the shadow of the reduction: this lane's row scaled by 1 / its candidate
+                const double linv = rcp_nr(t[b]);
+                double scl[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) scl[c] = (c == b) ? linv : t[c] * linv;
+                bool cand = !used_r && khi == mhi;
+                const unsigned ball = __ballot_sync(FULL, cand);
+                int src;
+                if (__popc(ball) == 1) {
+                    src = __ffs(ball) - 1;
+                } else { // ties in the high word (or no unused row in this warp): low words, then the lowest row
+                    const unsigned klo = (unsigned)key;
+                    const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
+                    cand = cand && klo == mlo;
+                    const unsigned b2 = __ballot_sync(FULL, cand);
+                    src = b2 ? __ffs(b2) - 1 : 0;
+                }
+                W2Slot *mys = &sh.slot[b & 1][w];
+                if (lane == src) {
+#pragma unroll
+                    for (int c = 0; c < FR_NB / 2; ++c)
+                        reinterpret_cast<double2 *>(mys->row)[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
+                    mys->key = key;
+                    mys->lane = lane;
+                }
+                __syncthreads(); // the two candidates of this step are visible (two slot buffers alternate)
+                const unsigned long long k0 = sh.slot[b & 1][0].key, k1 = sh.slot[b & 1][1].key;
+                const int gw = k1 > k0 ? 1 : 0; // a tie goes to warp 0: the lower row
+                const unsigned long long kmax = gw ? k1 : k0;
+                if ((unsigned)(kmax >> 32) == 0u || (unsigned)(kmax >> 32) >= 0x7ff00000u) bad = true; // zero / denormal / inf / NaN
+                const W2Slot *win = &sh.slot[b & 1][gw];
+                const int lw = win->lane;
+                Rl[b] = 32 * gw + lw;
+                double sp[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB / 2; ++c) {
+                    const double2 v = reinterpret_cast<const double2 *>(win->row)[c];
+                    sp[2 * c] = v.x;
+                    sp[2 * c + 1] = v.y;
+                }
+                const bool is_p = gw == w && lane == lw;
+                const double f = is_p ? 0.0 : t[b];
+                const double g = is_p ? linv : 1.0; // the pivot row becomes itself / pivot
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) {
+                    if (c == b) t[c] = is_p ? linv : -f * sp[b];
+                    else t[c] = fma(-f, sp[c], t[c] * g);
+                }
+                if (is_p) used_r = true;
+                if (threadIdx.x == b) { sh.rho[FR_NB * pnl + b] = Rl[b]; sh.rhoinv[Rl[b]] = FR_NB * pnl + b; }
+            }
+            // ---- publish Z = T[:, R] - I[:, R] and the eliminated panel; the owner's shadow of the panel columns becomes 0
+            // so that phase U leaves them alone
+#pragma unroll
+            for (int b = 0; b < FR_NB; ++b) {
+                sh.Z[b][r] = t[b] - (Rl[b] == r ? 1.0 : 0.0);
+                sh.Pn[b][r] = t[b];
+            }
+            if (owner) {
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) Sw[(8 * st + c) * 32 + lane] = make_double2(0.0, 0.0);
+            }
+            __syncthreads();
+            if (bad) { singular = true; break; } // uniform across the CTA
+            if (owner) { // the panel's own columns now hold T e_r
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (k == st) {
+#pragma unroll
+                        for (int c = 0; c < FR_NB; ++c) {
+                            const double2 v = *reinterpret_cast<const double2 *>(&sh.Pn[c][2 * lane]);
+                            a[8 * k + c][0] = v.x;
+                            a[8 * k + c][1] = v.y;
+                        }
+                    }
             }
 
             // ---- phase U: rank-8 update  a[:, c] += Z[:, b] * W_old[r_b, c]  of this lane's 2 x 32 tile
 #pragma unroll
             for (int b = 0; b < FR_NB; ++b) {
-                const double2 z = *reinterpret_cast<const double2 *>(&sh.Z[buf][b][2 * lane]);
-                const double *row = &sh.S[w][0][Rv[b]]; // W_old[r_b, local column c] at row[64 c] (uniform address)
+                const double2 z = *reinterpret_cast<const double2 *>(&sh.Z[b][2 * lane]);
+                const double *row = &sh.S[w][0][Rl[b]]; // W_old[r_b, local column c] at row[64 c] (uniform address)
 #pragma unroll
                 for (int c = 0; c < 32; ++c) {
                     const double rv = row[64 * c];
