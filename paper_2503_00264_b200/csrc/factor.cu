@@ -564,12 +564,11 @@ __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restr
                     sp[2 * c + 1] = v.y;
                 }
                 const bool is_p = gw == w && lane == lw;
-                const double f = is_p ? 0.0 : t[b];
-                const double g = is_p ? linv : 1.0; // the pivot row becomes itself / pivot
+                const double f = t[b];
 #pragma unroll
-                for (int c = 0; c < FR_NB; ++c) {
-                    if (c == b) t[c] = is_p ? linv : -f * sp[b];
-                    else t[c] = fma(-f, sp[c], t[c] * g);
+                for (int c = 0; c < FR_NB; ++c) { // the pivot row becomes itself / pivot (= scl, computed above)
+                    const double upd = (c == b) ? -f * sp[b] : fma(-f, sp[c], t[c]);
+                    t[c] = is_p ? scl[c] : upd;
                 }
                 if (is_p) used_r = true;
                 if (threadIdx.x == b) { sh.rho[FR_NB * pnl + b] = Rl[b]; sh.rhoinv[Rl[b]] = FR_NB * pnl + b; }
