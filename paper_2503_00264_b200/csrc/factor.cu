@@ -164,93 +164,17 @@ __device__ __forceinline__ double rcp_nr(double x)
     return fma(r, e, r);
 }
 
-// Phase P of the blocked Gauss-Jordan (both register-tiled kernels): one warp eliminates its n x 8 panel `a`
-// (lane l holds the rows {64 s + 2 l, 64 s + 2 l + 1}, s < TR / 2, register row rr = 2 s + e) with warp-level
-// operations only. usedmask: bit rr set = that row of this lane was a pivot row of an earlier step. Returns the pivot
-// rows in Rl and whether a zero / non-finite pivot was met.
-template <int TR>
-__device__ __forceinline__ bool panel_eliminate(double (&a)[TR][8], unsigned usedmask, int lane, int (&Rl)[FR_NB])
-{
-    constexpr unsigned FULL = 0xffffffffu;
-    // Everything that does not depend on WHICH row wins (1/candidate, the candidate row scaled by it)
-    // is computed by every lane for its own candidate in the shadow of the arg-max reduction; the
-    // winner's scaled row is then broadcast by shuffles.
-    bool bad = false;
-    unsigned um = usedmask;
-#pragma unroll
-    for (int b = 0; b < FR_NB; ++b) {
-        // local candidate: first row of maximal |entry| among this lane's unused rows
-        unsigned long long bk = 0ull;
-        int brr = -1;
-#pragma unroll
-        for (int rr = 0; rr < TR; ++rr) {
-            const unsigned long long key = (unsigned long long)__double_as_longlong(fabs(a[rr][b]));
-            if (!((um >> rr) & 1u) && (brr < 0 || key > bk)) { bk = key; brr = rr; }
-        }
-        const bool valid = brr >= 0;
-        const unsigned khi = valid ? (unsigned)(bk >> 32) : 0u;
-        const unsigned mhi = __reduce_max_sync(FULL, khi);
-        // (independent of the reduction) the candidate row, scaled by 1/candidate; column b holds 1/candidate
-        double scl[8];
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            double v = a[0][c];
-#pragma unroll
-            for (int rr = 1; rr < TR; ++rr) v = (brr == rr) ? a[rr][c] : v;
-            scl[c] = v;
-        }
-        const double linv = rcp_nr(scl[b]);
-#pragma unroll
-        for (int c = 0; c < 8; ++c) scl[c] = (c == b) ? linv : scl[c] * linv;
-        const unsigned bit0 = __ballot_sync(FULL, brr & 1), bit1 = __ballot_sync(FULL, brr & 2),
-                       bit2 = __ballot_sync(FULL, brr & 4);
-        // winner: the only lane whose high key word equals the maximum (common case), else exact
-        bool cand = valid && khi == mhi;
-        const unsigned ball = __ballot_sync(FULL, cand);
-        int src;
-        if (__popc(ball) == 1) {
-            src = __ffs(ball) - 1;
-        } else { // ties in the high word (or no valid row): compare the low words, then the lowest row
-            const unsigned klo = (unsigned)bk;
-            const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
-            cand = cand && klo == mlo;
-            const int row = cand ? 64 * (brr >> 1) + 2 * lane + (brr & 1) : INT_MAX;
-            const int rmin = __reduce_min_sync(FULL, row);
-            src = rmin == INT_MAX ? 0 : (rmin & 63) >> 1;
-        }
-        if (mhi == 0u || mhi >= 0x7ff00000u) bad = true; // zero / denormal, inf or NaN pivot
-        const int rr_r = (int)(((bit0 >> src) & 1u) | (((bit1 >> src) & 1u) << 1) | (((bit2 >> src) & 1u) << 2)) &
-                         (TR - 1); // warp-uniform
-        Rl[b] = 64 * (rr_r >> 1) + 2 * src + (rr_r & 1);
-        const bool mine = lane == src;
-        // pivot row (already scaled): broadcast from the winner's registers by shuffles -- no shared-memory round trip
-        // and no memory barrier in the instruction stream, so the trailing updates of this step can overlap the
-        // next step's arg-max
-        double sp[8];
-#pragma unroll
-        for (int c = 0; c < 8; ++c) sp[c] = __shfl_sync(FULL, scl[c], src);
-#pragma unroll
-        for (int rr = 0; rr < TR; ++rr) {
-            const bool is_p = mine && rr == rr_r;
-            const double f = is_p ? 0.0 : a[rr][b];
-            const double g = is_p ? linv : 1.0; // the pivot row becomes itself / pivot
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                if (c == b) {
-                    const double t = -f * sp[b];
-                    a[rr][c] = is_p ? linv : t;
-                } else {
-                    a[rr][c] = fma(-f, sp[c], a[rr][c] * g);
-                }
-            }
-        }
-        if (mine) um |= 1u << rr_r;
-    }
-    return bad;
-}
+struct PivotSlot {                 // what a warp's local arg-max winner publishes in a pivot step
+    double row[FR_NB];             // its panel row, scaled by 1 / candidate (column b holds 1 / candidate)
+    unsigned long long key;        // bit pattern of |candidate| (0: this warp has no unused row)
+    int lane;
+    int pad;
+};
 
 template <int NQ> struct FrShared {
     double Z[2][FR_NB][64 * NQ];          // [buf][b][row]
+    double Pn[FR_NB][64 * NQ];            // [c][row]: the panel, owner's registers -> one row per thread -> back
+    PivotSlot slot[2][FR_THREADS / 32];   // [step parity][warp]
     double Rrow[2][FR_NB][64];            // [buf][b][local column]
     int R[2][FR_NB];                      // pivot rows of the panel
     int sing[2];                          // panel met a zero / non-finite pivot
@@ -262,7 +186,9 @@ __global__ void __launch_bounds__(FR_THREADS, NQ == 1 ? 3 : (NQ == 2 ? 2 : 1))
 factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
 {
     constexpr int n = 64 * NQ, TR = 2 * NQ, NPANEL = n / FR_NB;
-    __shared__ __align__(16) FrShared<NQ> sh;
+    extern __shared__ __align__(16) unsigned char fr_smem[];
+    FrShared<NQ> &sh = *reinterpret_cast<FrShared<NQ> *>(fr_smem);
+    constexpr unsigned FULL = 0xffffffffu;
     cg::cluster_group cluster = cg::this_cluster();
     const int q = NQ == 1 ? 0 : (int)cluster.block_rank();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -323,45 +249,130 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
                 }
             }
         }
-        unsigned usedmask = 0;
+        bool used_r = false; // row threadIdx.x (the row this thread holds during panel phases) was a pivot row
         bool singular = false;
 
         for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
             const int buf = gp & 1;
-            const bool owner = (pnl >> 3) == q && (pnl & 7) == w;
-            if (owner) {
-                // ================= phase P: eliminate the n x 8 panel inside this warp =====================
+            const bool owner_cta = (pnl >> 3) == q;
+            const bool owner = owner_cta && (pnl & 7) == w;
+            if (owner_cta) {
+                // ================= phase P: the owner CTA eliminates the n x 8 panel, ONE ROW PER THREAD ==============
+                // (a warp holding TR rows per lane would run ~70 + 45 TR dependent instructions per pivot step alone)
+                __syncthreads(); // the previous panel's owner warp has read its panel back from Pn
+                if (owner) {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c)
+#pragma unroll
+                        for (int sq = 0; sq < NQ; ++sq)
+                            *reinterpret_cast<double2 *>(&sh.Pn[c][64 * sq + 2 * lane]) = make_double2(a[2 * sq][c], a[2 * sq + 1][c]);
+                }
+                __syncthreads();
+                const int r = threadIdx.x;             // this thread's row during the panel phase
+                const bool row_on = r < n;
+                double t[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) t[c] = row_on ? sh.Pn[c][r] : 0.0;
                 int Rl[FR_NB];
-                const bool bad = panel_eliminate<TR>(a, usedmask, lane, Rl);
-                // ---- publish Z = T[:, R] - I[:, R], R and the singular flag to every CTA of the cluster
+                bool bad = false;
+                bool used_p = used_r;
 #pragma unroll
-                for (int t = 0; t < NQ; ++t) {
-                    FrShared<NQ> *dst = NQ == 1 ? &sh : cluster.map_shared_rank(&sh, t);
+                for (int b = 0; b < FR_NB; ++b) {
+                    const unsigned long long key =
+                        (used_p || !row_on) ? 0ull : (unsigned long long)__double_as_longlong(fabs(t[b]));
+                    const unsigned khi = (unsigned)(key >> 32);
+                    const unsigned mhi = __reduce_max_sync(FULL, khi);
+                    const double linv = rcp_nr(t[b]);
+                    double scl[FR_NB];
 #pragma unroll
-                    for (int b = 0; b < FR_NB; ++b) {
-#pragma unroll
-                        for (int s = 0; s < NQ; ++s) {
-                            const int row0 = 64 * s + 2 * lane;
-                            double2 z;
-                            z.x = a[2 * s][b] - (Rl[b] == row0 ? 1.0 : 0.0);
-                            z.y = a[2 * s + 1][b] - (Rl[b] == row0 + 1 ? 1.0 : 0.0);
-                            *reinterpret_cast<double2 *>(&dst->Z[buf][b][row0]) = z;
-                        }
-                        if (lane == b) dst->R[buf][b] = Rl[b];
+                    for (int c = 0; c < FR_NB; ++c) scl[c] = (c == b) ? linv : t[c] * linv;
+                    bool cand = !used_p && row_on && khi == mhi;
+                    const unsigned ball = __ballot_sync(FULL, cand);
+                    int src;
+                    if (__popc(ball) == 1) {
+                        src = __ffs(ball) - 1;
+                    } else { // ties in the high word (or no unused row in this warp): low words, then the lowest row
+                        const unsigned klo = (unsigned)key;
+                        const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
+                        cand = cand && klo == mlo;
+                        const unsigned b2 = __ballot_sync(FULL, cand);
+                        src = b2 ? __ffs(b2) - 1 : 0;
                     }
-                    if (lane == 0) dst->sing[buf] = bad ? 1 : 0;
+                    PivotSlot *mys = &sh.slot[b & 1][w];
+                    if (lane == src) {
+#pragma unroll
+                        for (int c = 0; c < FR_NB / 2; ++c)
+                            reinterpret_cast<double2 *>(mys->row)[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
+                        mys->key = key;
+                        mys->lane = lane;
+                    }
+                    __syncthreads(); // the candidates of this step are visible (two slot buffers alternate)
+                    unsigned long long kmax = sh.slot[b & 1][0].key;
+                    int gw = 0;
+#pragma unroll
+                    for (int ww = 1; ww < n / 32; ++ww) { // a tie goes to the lower warp: the lower row
+                        const unsigned long long kk = sh.slot[b & 1][ww].key;
+                        if (kk > kmax) { kmax = kk; gw = ww; }
+                    }
+                    if ((unsigned)(kmax >> 32) == 0u || (unsigned)(kmax >> 32) >= 0x7ff00000u) bad = true;
+                    const PivotSlot *win = &sh.slot[b & 1][gw];
+                    const int lw = win->lane;
+                    Rl[b] = 32 * gw + lw;
+                    double sp[FR_NB];
+#pragma unroll
+                    for (int c = 0; c < FR_NB / 2; ++c) {
+                        const double2 v = reinterpret_cast<const double2 *>(win->row)[c];
+                        sp[2 * c] = v.x;
+                        sp[2 * c + 1] = v.y;
+                    }
+                    const bool is_p = gw == w && lane == lw;
+                    const double f = t[b];
+#pragma unroll
+                    for (int c = 0; c < FR_NB; ++c) {
+                        const double upd = (c == b) ? -f * sp[b] : fma(-f, sp[c], t[c]);
+                        t[c] = is_p ? scl[c] : upd;
+                    }
+                    if (is_p) used_p = true;
+                }
+                // ---- publish Z = T[:, R] - I[:, R], R and the singular flag to every CTA of the cluster; the eliminated
+                // panel goes back to its owner warp through Pn
+#pragma unroll
+                for (int tq = 0; tq < NQ; ++tq) {
+                    FrShared<NQ> *dst = NQ == 1 ? &sh : cluster.map_shared_rank(&sh, tq);
+                    if (row_on) {
+#pragma unroll
+                        for (int b = 0; b < FR_NB; ++b) dst->Z[buf][b][r] = t[b] - (Rl[b] == r ? 1.0 : 0.0);
+                    }
+#pragma unroll
+                    for (int b = 0; b < FR_NB; ++b)
+                        if (threadIdx.x == b) dst->R[buf][b] = Rl[b];
+                    if (threadIdx.x == 0) dst->sing[buf] = bad ? 1 : 0;
+                }
+                if (row_on) {
+#pragma unroll
+                    for (int c = 0; c < FR_NB; ++c) sh.Pn[c][r] = t[c];
                 }
             }
             cluster_barrier(); // B1: Z, R, sing of this panel visible everywhere
 
             if (sh.sing[buf]) { singular = true; ++gp; break; } // uniform across the cluster
+            if (owner) { // the panel's own columns now hold T e_r
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+#pragma unroll
+                    for (int sq = 0; sq < NQ; ++sq) {
+                        const double2 v = *reinterpret_cast<const double2 *>(&sh.Pn[c][64 * sq + 2 * lane]);
+                        a[2 * sq][c] = v.x;
+                        a[2 * sq + 1][c] = v.y;
+                    }
+            }
             // ---- every thread: note the pivot rows; holders publish the OLD entries of their pivot rows
 #pragma unroll
             for (int b = 0; b < FR_NB; ++b) {
                 const int r = sh.R[buf][b];
                 const int lane_r = (r & 63) >> 1, rr_r = 2 * (r >> 6) + (r & 1);
+                if (r == (int)threadIdx.x) used_r = true;
                 if (lane == lane_r) {
-                    usedmask |= 1u << rr_r;
                     if (!owner) {
                         double2 *dst = reinterpret_cast<double2 *>(&sh.Rrow[buf][b][8 * w]);
 #pragma unroll
@@ -434,18 +445,11 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
 // to its owner's registers, and both warps apply the rank-8 update to their 32 columns.
 constexpr int W2_THREADS = 64;
 
-struct W2Slot {                    // what a warp's local arg-max winner publishes in a pivot step
-    double row[FR_NB];             // its panel row, scaled by 1 / candidate (column b holds 1 / candidate)
-    unsigned long long key;        // bit pattern of |candidate| (0: this warp has no unused row)
-    int lane;
-    int pad;
-};
-
 struct W2Shared {
     double S[2][32][64];           // [warp][local column][row]: shadow copy of the warp's tile, refreshed every panel
     double Z[FR_NB][64];           // [b][row]
     double Pn[FR_NB][64];          // [c][row]: the eliminated panel on its way back to the owner's registers
-    W2Slot slot[2][2];             // [step parity][warp]
+    PivotSlot slot[2][2];             // [step parity][warp]
     int rho[64], rhoinv[64];
 };
 
@@ -540,7 +544,7 @@ __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restr
                     const unsigned b2 = __ballot_sync(FULL, cand);
                     src = b2 ? __ffs(b2) - 1 : 0;
                 }
-                W2Slot *mys = &sh.slot[b & 1][w];
+                PivotSlot *mys = &sh.slot[b & 1][w];
                 if (lane == src) {
 #pragma unroll
                     for (int c = 0; c < FR_NB / 2; ++c)
@@ -553,7 +557,7 @@ __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restr
                 const int gw = k1 > k0 ? 1 : 0; // a tie goes to warp 0: the lower row
                 const unsigned long long kmax = gw ? k1 : k0;
                 if ((unsigned)(kmax >> 32) == 0u || (unsigned)(kmax >> 32) >= 0x7ff00000u) bad = true; // zero / denormal / inf / NaN
-                const W2Slot *win = &sh.slot[b & 1][gw];
+                const PivotSlot *win = &sh.slot[b & 1][gw];
                 const int lw = win->lane;
                 Rl[b] = 32 * gw + lw;
                 double sp[FR_NB];
@@ -665,7 +669,9 @@ template <int NQ> static int launch_factor_reg(oci_ctx *ctx, const ProblemView &
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.blockDim = dim3(FR_THREADS, 1, 1);
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = sizeof(FrShared<NQ>);
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_reg_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)sizeof(FrShared<NQ>)));
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -680,7 +686,8 @@ template <int NQ> static int launch_factor_reg(oci_ctx *ctx, const ProblemView &
         OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_reg_kernel<NQ>, &cfg));
     } else {
         int per_sm = 0;
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_reg_kernel<NQ>, FR_THREADS, 0));
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_reg_kernel<NQ>, FR_THREADS,
+                                                                        sizeof(FrShared<NQ>)));
         n_clusters = per_sm * ctx->num_sms;
     }
     if (n_clusters < 1) n_clusters = 1;
