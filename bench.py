@@ -49,8 +49,8 @@ UNIT = "cell-solves/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of one oci_iterate_wpc_kernel<2,0> launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/r01_c_ncu_full.md (2.214779 GB read + 38.01 MB written).
 NCU_TRAFFIC_BYTES_PER_LAUNCH = 2252789624
-# same for one factor launch (factor_w2_kernel): 2.07 MB read + 2.097311 GB written
-NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2099381528
+# same for one factor launch (factor_w2_kernel, profiles/r01_e_factor.md)
+NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2090512639
 # same for one st_iterate_pipe_kernel<0,1> launch (profiles/r01_d_ncu_full.md): 213.30 MB read + 21.86 MB written
 NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH = 235150848
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
