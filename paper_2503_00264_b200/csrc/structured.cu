@@ -295,17 +295,15 @@ __global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterPar
 // the layouts) into a ring of `stages` shared-memory stages guarded by mbarriers, so that HBM stays busy while the
 // 256 consumer threads work out of shared memory. The blocks are re-read from shared memory for x = z + D^-1 U y
 // instead of being held in registers across the barriers.
-constexpr int STP_CONSUMERS = ST_THREADS;
-constexpr int STP_THREADS = ST_THREADS + 32;
 constexpr int STP_MAX_STAGES = 6;
 
 struct StStage {                // element offsets inside one stage (all multiples of 2 doubles)
     int Lt, cs, nb, Ci, doubles;
 };
 
-__host__ __device__ inline StStage st_stage_layout(int N, int G)
+__host__ __device__ inline StStage st_stage_layout(int N, int G, int CT)
 {
-    const int GN = G * N, n = 4 * GN, G4 = 4 * G, CPB = ST_THREADS / GN;
+    const int GN = G * N, n = 4 * GN, G4 = 4 * G, CPB = CT / GN;
     StStage s;
     s.Lt = 0;
     s.cs = s.Lt + CPB * 16 * GN;
@@ -315,15 +313,17 @@ __host__ __device__ inline StStage st_stage_layout(int N, int G)
     return s;
 }
 
-template <bool WANT_L2, int GC>
-__global__ void __launch_bounds__(STP_THREADS, 2) st_iterate_pipe_kernel(const IterParams P, const StParams S, int stages)
+// CT = consumer threads per CTA (256, or 128 so that four CTAs share an SM); one more warp holds the producer thread.
+template <bool WANT_L2, int GC, int CT>
+__global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_kernel(const IterParams P, const StParams S, int stages)
 {
     if (stop_reached(P.stop)) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
     extern __shared__ __align__(128) unsigned char stp_smem[];
     const int N = P.N, G = GC > 0 ? GC : P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
-    const int CPB = ST_THREADS / GN;
-    const StStage lay = st_stage_layout(N, G);
+    constexpr int STP_CONSUMERS = CT, STP_THREADS = CT + 32;
+    const int CPB = CT / GN;
+    const StStage lay = st_stage_layout(N, G, CT);
     uint64_t *full = reinterpret_cast<uint64_t *>(stp_smem);
     uint64_t *empty = full + STP_MAX_STAGES;
     double *mu_s = reinterpret_cast<double *>(empty + STP_MAX_STAGES); // [N]
@@ -572,14 +572,18 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
 {
     StParams S;
     S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
-    const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
+    const int GN = ctx->G * ctx->N, G4 = 4 * ctx->G;
     if (ctx->opt_iterate_kernel == 1) { // persistent bulk-copy pipeline; falls through when the ring would not fit
-        const StStage lay = st_stage_layout(ctx->N, ctx->G);
+        // 256 consumer threads and two CTAs per SM; 128 and four when a cell takes a whole warp (measured: config 3,
+        // G N = 32, 16.5 -> 13.4 us per iteration; config 5, G N = 16, is faster with 256: 45 against 47 us)
+        const int CT = (GN > 16 && GN <= 32 && ctx->opt_ctas_per_sm != 2) ? 128 : 256, CPB = CT / GN;
+        const int max_ctas = CT == 128 ? 4 : 2;
+        const StStage lay = st_stage_layout(ctx->N, ctx->G, CT);
         const size_t fixed = (size_t)2 * STP_MAX_STAGES * 8 + sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 +
                                                                                (size_t)3 * CPB * G4) + 256;
         // two CTAs per SM by default: each is a lock-step sequence of short latency-bound phases, two of them overlap
-        int ctas = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : 2;
-        if (ctas > 2) ctas = 2;
+        int ctas = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : max_ctas;
+        if (ctas > max_ctas) ctas = max_ctas;
         int stages = 0;
         for (; ctas >= 1; --ctas) {
             const size_t budget = ((size_t)ctx->max_smem_optin + 1024) / ctas - 1024; // 228 KB per SM, 1 KB reserved per CTA
@@ -593,20 +597,25 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
             const size_t smem = fixed + (size_t)stages * lay.doubles * 8;
             int grid = ctx->num_sms * ctas;
             if (grid > (ctx->J + CPB - 1) / CPB) grid = (ctx->J + CPB - 1) / CPB;
-#define OCI_STP_LAUNCH(L2_, GC_)                                                                                   \
+#define OCI_STP_LAUNCH(L2_, GC_, CT_)                                                                              \
     do {                                                                                                           \
         static size_t attr = 0;                                                                                    \
         if (attr < smem) {                                                                                         \
-            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(st_iterate_pipe_kernel<L2_, GC_>,                               \
+            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(st_iterate_pipe_kernel<L2_, GC_, CT_>,                          \
                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
             attr = smem;                                                                                           \
         }                                                                                                          \
-        st_iterate_pipe_kernel<L2_, GC_><<<grid, STP_THREADS, smem, ctx->stream>>>(P, S, stages);                  \
+        st_iterate_pipe_kernel<L2_, GC_, CT_><<<grid, CT_ + 32, smem, ctx->stream>>>(P, S, stages);                \
     } while (0)
 #define OCI_STP_G(GC_)                                                                                             \
     do {                                                                                                           \
-        if (want_l2) OCI_STP_LAUNCH(true, GC_);                                                                    \
-        else OCI_STP_LAUNCH(false, GC_);                                                                           \
+        if (CT == 128) {                                                                                           \
+            if (want_l2) OCI_STP_LAUNCH(true, GC_, 128);                                                           \
+            else OCI_STP_LAUNCH(false, GC_, 128);                                                                  \
+        } else {                                                                                                   \
+            if (want_l2) OCI_STP_LAUNCH(true, GC_, 256);                                                           \
+            else OCI_STP_LAUNCH(false, GC_, 256);                                                                  \
+        }                                                                                                          \
     } while (0)
             switch (ctx->G) {
             case 1: OCI_STP_G(1); break;
@@ -621,6 +630,7 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
             return 1;
         }
     }
+    const int CPB = ST_THREADS / GN;
     const size_t smem = sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 + (size_t)3 * CPB * G4);
     const int grid = (ctx->J + CPB - 1) / CPB; // one batch of CPB cells per CTA: CTA turnover hides the load latency
 #define OCI_ST_LAUNCH(GC_)                                                                                         \
