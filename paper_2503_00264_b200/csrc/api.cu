@@ -89,6 +89,9 @@ size_t carve(oci_ctx *c, unsigned char *base, int J, int N, int G, int num_sms, 
     const size_t GNpad = (GN + 15) / 16 * 16; // room for any "si_lanes" grouping (4, 8, 16)
     t->si_T2sw = cv.take<double>((size_t)J * GNpad * 4);
     t->si_bsw = cv.take<double>((size_t)J * GNpad * 2);
+    // scan mode: 6 doubles per thread prefix (one thread per 4 sweep steps) + per 1024-step block aggregate, per chain
+    t->si_scan_bytes = (((size_t)J + 1023) / 1024) * GN * 257 * 6 * sizeof(double);
+    t->si_scan = cv.take<double>(t->si_scan_bytes / sizeof(double));
     t->st_LinvT = cv.take<double>((size_t)J * GN * 16);
     t->st_Wg = cv.take<double>((size_t)J * G * 16);
     t->st_Cinv = cv.take<double>((size_t)J * 16 * G * G);
@@ -373,6 +376,11 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
         if (value == 1 && !st_supported(ctx)) return OCI_E_UNSUPPORTED;
         if ((int)value != ctx->opt_solve_mode) ctx->factored = false;
         ctx->opt_solve_mode = (int)value;
+    }
+    else if (!strcmp(key, "si_sweep")) {
+        if (value != 0 && value != 1) return -3;
+        if ((int)value != ctx->opt_si_sweep) ctx->si_valid = false; // the sweep-order arrays change layout
+        ctx->opt_si_sweep = (int)value;
     }
     else if (!strcmp(key, "si_lanes")) { ctx->opt_si_lanes = (int)value; ctx->si_valid = false; }
     else return -2;

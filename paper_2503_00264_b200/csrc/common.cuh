@@ -49,6 +49,8 @@ struct oci_ctx {
     double *si_in;      // [J][G*N][2]    incident edge flux of cell j found by the sweep
     double *si_T2sw;    // [ceil(GN/lpc)][J][lpc][2][2]  incident -> outgoing 2x2 map, sweep order (si.cu sweep_index)
     double *si_bsw;     // [ceil(GN/lpc)][J][lpc][2]     outgoing entries of si_base, sweep order
+    double *si_scan;    // scan mode ("si_sweep" = 1): per-thread prefixes and per-block aggregates (si.cu)
+    size_t si_scan_bytes;
     // structured cell solve ("solve_mode" = 1; structured.cu)
     double *st_LinvT;   // [J][16][G*N]   L_{c,j,g,m}^-1, ordinate-fastest
     double *st_Wg;      // [J][G][16]     sum_m w_m L^-1_{j,g,m}
@@ -66,7 +68,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];

@@ -256,6 +256,134 @@ __global__ void __launch_bounds__(SW_THREADS) si_sweep_kernel(StopCheck stop, in
     }
 }
 
+// ============================================================================================================
+// SURVEY 8(f) row f4 (second half): the sweep as a parallel scan -- "si_sweep" = 1. NOT the comparator of north_star
+// (which is serial in space, above); it is here because it changes the OCI-vs-SI verdict and that should be known.
+// ============================================================================================================
+// The per-cell maps in -> T in + b are affine, and composition of affine maps is associative, so the incident flux of
+// every cell is a prefix "sum" under composition along the sweep direction. Two kernels, no inter-CTA waiting:
+//   si_scan_reduce : per (chain, block of 1024 sweep steps): every thread composes its 4 maps, a block-level scan
+//                    (shuffles + shared memory) gives each thread the composition of everything before it in the
+//                    block (stored) and the block its aggregate (stored);
+//   si_scan_apply  : every block folds the aggregates of the blocks before it onto the boundary value (<= J / 1024 short
+//                    steps), every thread applies its stored prefix and walks its 4 cells.
+// Layout: the sweep-order arrays with lpc = 1, i.e. chain-major, so consecutive threads read consecutive cells.
+constexpr int SCAN_THREADS = 256, SCAN_PER_THREAD = 4, SCAN_BLOCK = SCAN_THREADS * SCAN_PER_THREAD;
+
+struct Affine {            // x -> M x + c, M = [[m00, m01], [m10, m11]]
+    double m00, m01, m10, m11, c0, c1;
+};
+__device__ __forceinline__ Affine affine_identity() { return Affine{1.0, 0.0, 0.0, 1.0, 0.0, 0.0}; }
+// second after first: x -> second(first(x))
+__device__ __forceinline__ Affine affine_then(const Affine &first, const Affine &second)
+{
+    Affine r;
+    r.m00 = fma(second.m00, first.m00, second.m01 * first.m10);
+    r.m01 = fma(second.m00, first.m01, second.m01 * first.m11);
+    r.m10 = fma(second.m10, first.m00, second.m11 * first.m10);
+    r.m11 = fma(second.m10, first.m01, second.m11 * first.m11);
+    r.c0 = fma(second.m00, first.c0, fma(second.m01, first.c1, second.c0));
+    r.c1 = fma(second.m10, first.c0, fma(second.m11, first.c1, second.c1));
+    return r;
+}
+__device__ __forceinline__ Affine affine_shfl_up(const Affine &a, int d)
+{
+    Affine r;
+    r.m00 = __shfl_up_sync(0xffffffffu, a.m00, d); r.m01 = __shfl_up_sync(0xffffffffu, a.m01, d);
+    r.m10 = __shfl_up_sync(0xffffffffu, a.m10, d); r.m11 = __shfl_up_sync(0xffffffffu, a.m11, d);
+    r.c0 = __shfl_up_sync(0xffffffffu, a.c0, d);   r.c1 = __shfl_up_sync(0xffffffffu, a.c1, d);
+    return r;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS)
+si_scan_reduce_kernel(StopCheck stop, int J, const double *__restrict__ T2, const double *__restrict__ bo,
+                      Affine *__restrict__ prefix, Affine *__restrict__ agg)
+{
+    __shared__ Affine wagg[SCAN_THREADS / 32];
+    if (stop_reached(stop)) return;
+    const int ch = blockIdx.y, blk = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_blk = gridDim.x;
+    const size_t jj0 = (size_t)blk * SCAN_BLOCK + (size_t)tid * SCAN_PER_THREAD;
+    const double *Tp = T2 + ((size_t)ch * J + jj0) * 4;
+    const double *bp = bo + ((size_t)ch * J + jj0) * 2;
+    Affine a = affine_identity();
+#pragma unroll
+    for (int u = 0; u < SCAN_PER_THREAD; ++u)
+        if (jj0 + u < (size_t)J) {
+            const double2 t0 = *reinterpret_cast<const double2 *>(Tp + 4 * u);
+            const double2 t1 = *reinterpret_cast<const double2 *>(Tp + 4 * u + 2);
+            const double2 bb = *reinterpret_cast<const double2 *>(bp + 2 * u);
+            a = affine_then(a, Affine{t0.x, t0.y, t1.x, t1.y, bb.x, bb.y});
+        }
+    // inclusive scan inside the warp (Hillis-Steele under composition: earlier lanes act first)
+    Affine inc = a;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const Affine up = affine_shfl_up(inc, d);
+        if (lane >= d) inc = affine_then(up, inc);
+    }
+    if (lane == 31) wagg[warp] = inc;
+    Affine exc = affine_shfl_up(inc, 1);
+    if (lane == 0) exc = affine_identity();
+    __syncthreads();
+    Affine wpre = affine_identity();
+    for (int ww = 0; ww < warp; ++ww) wpre = affine_then(wpre, wagg[ww]);
+    const Affine pre = affine_then(wpre, exc);              // everything before this thread, inside the block
+    prefix[((size_t)ch * n_blk + blk) * SCAN_THREADS + tid] = pre;
+    if (tid == SCAN_THREADS - 1) agg[(size_t)ch * n_blk + blk] = affine_then(pre, a);
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS)
+si_scan_apply_kernel(StopCheck stop, int J, int N, int G, int bc_left, int bc_right, const double *__restrict__ mu,
+                     const double *__restrict__ T2, const double *__restrict__ bo, const Affine *__restrict__ prefix,
+                     const Affine *__restrict__ agg, const double *__restrict__ psi_old,
+                     const double *__restrict__ inc_left, const double *__restrict__ inc_right,
+                     double *__restrict__ in_out)
+{
+    if (stop_reached(stop)) return;
+    const int gm = blockIdx.y, blk = blockIdx.x, tid = threadIdx.x, n_blk = gridDim.x;
+    const int GN = G * N, n = 4 * GN, g = gm / N, m = gm % N;
+    const bool fwd = mu[m] > 0.0;
+    double x0 = 0.0, x1 = 0.0;
+    const int bc = fwd ? bc_left : bc_right;
+    if (bc == OCI_BC_REFLECTIVE) { // mirror ordinate of the boundary cell, from iteration l (A12)
+        const double *cellp = psi_old + (fwd ? (size_t)0 : (size_t)(J - 1) * n) + (size_t)(g * N + (N - 1 - m)) * 4;
+        x0 = cellp[fwd ? 0 : 1];
+        x1 = cellp[fwd ? 2 : 3];
+    } else if (bc == OCI_BC_PRESCRIBED) {
+        const double *ip = (fwd ? inc_left : inc_right) + (size_t)gm * 2;
+        x0 = ip[0];
+        x1 = ip[1];
+    }
+    for (int b = 0; b < blk; ++b) { // the blocks before this one (uniform loads)
+        const Affine A = agg[(size_t)gm * n_blk + b];
+        const double y0 = fma(A.m00, x0, fma(A.m01, x1, A.c0)), y1 = fma(A.m10, x0, fma(A.m11, x1, A.c1));
+        x0 = y0;
+        x1 = y1;
+    }
+    {
+        const Affine Pf = prefix[((size_t)gm * n_blk + blk) * SCAN_THREADS + tid];
+        const double y0 = fma(Pf.m00, x0, fma(Pf.m01, x1, Pf.c0)), y1 = fma(Pf.m10, x0, fma(Pf.m11, x1, Pf.c1));
+        x0 = y0;
+        x1 = y1;
+    }
+    const size_t jj0 = (size_t)blk * SCAN_BLOCK + (size_t)tid * SCAN_PER_THREAD;
+    const double *Tp = T2 + ((size_t)gm * J + jj0) * 4;
+    const double *bp = bo + ((size_t)gm * J + jj0) * 2;
+#pragma unroll
+    for (int u = 0; u < SCAN_PER_THREAD; ++u)
+        if (jj0 + u < (size_t)J) {
+            const size_t jj = jj0 + u, j = fwd ? jj : (size_t)(J - 1) - jj;
+            *reinterpret_cast<double2 *>(in_out + (j * GN + gm) * 2) = make_double2(x0, x1);
+            const double2 t0 = *reinterpret_cast<const double2 *>(Tp + 4 * u);
+            const double2 t1 = *reinterpret_cast<const double2 *>(Tp + 4 * u + 2);
+            const double2 bb = *reinterpret_cast<const double2 *>(bp + 2 * u);
+            const double y0 = fma(t0.x, x0, fma(t0.y, x1, bb.x)), y1 = fma(t1.x, x0, fma(t1.y, x1, bb.y));
+            x0 = y0;
+            x1 = y1;
+        }
+}
+
 // a11 (+ the rest of a10): psi = base + C in for every (j,g,m); phi = sum_m w_m psi_m; residual.
 constexpr int FIN_THREADS = 256;
 template <bool WANT_L2>
@@ -321,6 +449,7 @@ inline int grid_for(size_t total, int threads, int num_sms)
 // chains (ordinates x groups) per sweep CTA: 4, 8 or 16 ("si_lanes" option; default 8)
 static int si_lanes(const oci_ctx *ctx)
 {
+    if (ctx->opt_si_sweep == 1) return 1; // scan mode: chain-major layout
     const int v = ctx->opt_si_lanes;
     return (v == 4 || v == 16) ? v : 8;
 }
@@ -347,6 +476,19 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_pr
                                                                                    ctx->phi, ctx->si_Linv, ctx->si_base,
                                                                                    ctx->si_bsw);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
+    if (ctx->opt_si_sweep == 1) { // f4: the sweep as a parallel scan of the affine edge maps
+        const int n_blk = (ctx->J + SCAN_BLOCK - 1) / SCAN_BLOCK;
+        if ((size_t)n_blk * GN * (SCAN_THREADS + 1) * sizeof(Affine) > ctx->si_scan_bytes) return OCI_E_WORKSPACE;
+        Affine *prefix = reinterpret_cast<Affine *>(ctx->si_scan);
+        Affine *agg = prefix + (size_t)n_blk * GN * SCAN_THREADS;
+        const dim3 grid(n_blk, GN);
+        si_scan_reduce_kernel<<<grid, SCAN_THREADS, 0, ctx->stream>>>(stop, ctx->J, ctx->si_T2sw, ctx->si_bsw, prefix, agg);
+        OCI_CUDA_TRY(ctx, cudaGetLastError());
+        si_scan_apply_kernel<<<grid, SCAN_THREADS, 0, ctx->stream>>>(stop, ctx->J, ctx->N, ctx->G, ctx->bc_left,
+                                                                    ctx->bc_right, ctx->mu, ctx->si_T2sw, ctx->si_bsw, prefix,
+                                                                    agg, psi, ctx->inc_left, ctx->inc_right, ctx->si_in);
+        OCI_CUDA_TRY(ctx, cudaGetLastError());
+    } else {
     const int sweep_grid = (GN + lpc - 1) / lpc;
 #define OCI_SWEEP(LPC_)                                                                                            \
     do {                                                                                                           \
@@ -366,6 +508,7 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_pr
     else OCI_SWEEP(16);
 #undef OCI_SWEEP
     OCI_CUDA_TRY(ctx, cudaGetLastError());
+    }
     const int pairs_per_block = FIN_THREADS / ctx->N;
     size_t blocks = ((size_t)ctx->J * ctx->G + pairs_per_block - 1) / pairs_per_block;
     if (blocks > (size_t)ctx->num_sms * 16) blocks = (size_t)ctx->num_sms * 16;
@@ -380,5 +523,5 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_pr
                                                                              ctx->resid_inf + hist_slot,
                                                                              ctx->resid_l2 + hist_slot);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
-    return 3;
+    return ctx->opt_si_sweep == 1 ? 4 : 3;
 }

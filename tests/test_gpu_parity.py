@@ -376,3 +376,27 @@ def test_structured_mode_switch_refactors_and_flags_singular():
     p.sigma_t = p.sigma_t.copy()
     p.sigma_t[7] = np.nan
     assert _solver(p, options=ST).factor() == 8
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the SI sweep evaluated as a parallel scan ("si_sweep" = 1). Same oracle (serial sweep).
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES + [(13, 2500, 4, 2, 1, 2), (14, 1024, 8, 1, 0, 0)])
+def test_si_scan_per_iteration_parity(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p, options={"si_sweep": 1}), _oracle(p)
+    for l in range(4):
+        s.si_iterate(1)
+        o.si_iterate(1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+
+
+def test_si_scan_full_size_step_cfg5():
+    p = W.config5(dt=1e-2)
+    s, o = _solver(p, options={"si_sweep": 1}), _oracle(p)
+    it_g, conv_g, _ = s.si_step(tol=p.tol, max_iters=4000, check_every=8)
+    it_o, _ = o.si_step(tol=p.tol, max_iters=4000)
+    assert it_g == conv_g == it_o
+    assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+    assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
