@@ -293,6 +293,17 @@ def run_ours(args):
         per_dt[dt].setdefault("si_iters", []).append(it)
         per_dt[dt].setdefault("si_ms", []).append(el)
     diff = None if args.no_si else float((oci.scalar_flux() - si.scalar_flux()).abs().max().item())
+    # the same SI iteration with the sweep evaluated as a parallel scan (NOT north_star's comparator)
+    if not args.no_si:
+        si2 = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}", options={"si_sweep": 1})
+        for i in range(Wm + K):
+            dt = SWEEP[i % len(SWEEP)]
+            si2.set_dt(dt)
+            torch.cuda.synchronize(); t = time.perf_counter()
+            si2.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+            if i >= Wm:
+                per_dt[dt].setdefault("si_scan_ms", []).append((time.perf_counter() - t) * 1e3)
+        del si2
 
     # ---- end-to-end leg: host buffers through oci_step_host, copies inside the timed region ------------------
     e2e = OCISolver(p, dt=SWEEP[0], device=f"cuda:{local}")
@@ -371,7 +382,8 @@ def run_ours(args):
                       "oci_iter_kernel_ms": statistics.mean(d["iter_kernel_ms"]),
                       "structured_iters": d.get("st_iters"),
                       "structured_ms_per_step": statistics.mean(d["st_ms"]) if d.get("st_ms") else None,
-                      "si_ms_per_step": statistics.mean(d["si_ms"]) if d.get("si_ms") else None})
+                      "si_ms_per_step": statistics.mean(d["si_ms"]) if d.get("si_ms") else None,
+                      "si_scan_variant_ms_per_step": statistics.mean(d["si_scan_ms"]) if d.get("si_scan_ms") else None})
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
