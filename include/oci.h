@@ -95,7 +95,9 @@ int oci_last_cuda_error(const oci_ctx *ctx);
  * a1+a2 at the start of every step as Alg. 2 prints it; 0 [default] = only when dt changed), "si_lanes" (ordinates x
  * groups swept by one CTA of the SI sweep kernel: 4, 8 [default] or 16), "si_sweep" (0 = serial in space [default],
  * the comparator north_star names; 1 = the same sweep evaluated as a parallel scan of the per-cell affine edge maps,
- * same iterates to rounding). Returns -2 for an unknown key, -3 for a bad value. */
+ * same iterates to rounding), "persistent" (structured path only: -1 [default] = run a batch
+ * of iterations as ONE cooperative launch with grid-wide barriers when the problem is small (<= 8 MB per iteration),
+ * 0 = never, 1 = always). Returns -2 for an unknown key, -3 for a bad value. */
 int oci_set_option(oci_ctx *ctx, const char *key, int64_t value);
 
 int oci_set_dt(oci_ctx *ctx, double dt);                               /* invalidates the factors      */

@@ -140,6 +140,23 @@ int one_iteration(oci_ctx *ctx, int scheme, int slot, bool want_l2, bool check_p
                        : launch_si_iteration(ctx, slot, want_l2, check_prev);
 }
 
+// Iterations slot0 .. slot0 + k - 1 of one scheme; check_between: every iteration but the first looks at the residual of
+// the one before it and skips itself once the stop rule held (device-side stop). Returns kernels launched.
+int issue_batch(oci_ctx *ctx, int scheme, int slot0, int k, bool want_l2, bool check_between)
+{
+    if (scheme == 0) {
+        const int r = launch_st_multi(ctx, slot0, k, want_l2, check_between); // one cooperative launch, if it applies
+        if (r != 0) return r;
+    }
+    int launches = 0;
+    for (int i = 0; i < k; ++i) {
+        const int r = one_iteration(ctx, scheme, slot0 + i, want_l2, check_between && i > 0);
+        if (r < 0) return r;
+        launches += r;
+    }
+    return launches;
+}
+
 // The stop rule on the host: slot l of the history h (rule 0: max|dphi|; rule 1: sums of squares). Same arithmetic,
 // operation by operation, as stop_reached() on the device.
 bool rule_holds(int rule, double tol, const double *h_inf, const double *h_l2, int l)
@@ -167,11 +184,9 @@ int iterate_impl(oci_ctx *ctx, int scheme, int n_iters)
     if (n_iters > OCI_RESID_CAP) return -2;
     const int which = scheme == 0 ? 1 : 2;
     OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-    for (int i = 0; i < n_iters; ++i) {
-        r = one_iteration(ctx, scheme, ctx->hist_len + i, false, false);
-        if (r < 0) return r;
-        launches += r;
-    }
+    r = issue_batch(ctx, scheme, ctx->hist_len, n_iters, false, false);
+    if (r < 0) return r;
+    launches += r;
     OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     ctx->hist_len += n_iters;
     ctx->last_ms[which] = -1.0; // resolved lazily by oci_last_timing
@@ -215,12 +230,10 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
     while (it < max_iters && !conv_at) {
         const int k = (max_iters - it < check_every) ? max_iters - it : check_every;
         OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-        for (int i = 0; i < k; ++i) {
-            // slot it + i > it looks at slot it + i - 1 on the device and skips itself once the rule held
-            r = one_iteration(ctx, scheme, it + i, want_l2, i > 0);
-            if (r < 0) return r;
-            launches += r;
-        }
+        // slot it + i > it looks at slot it + i - 1 on the device and skips itself once the rule held
+        r = issue_batch(ctx, scheme, it, k, want_l2, true);
+        if (r < 0) return r;
+        launches += r;
         OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
         // the one host round-trip: k residuals + the executed-iterations counter, once every k iterations
         OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_inf + it, ctx->resid_inf + it, sizeof(double) * k, cudaMemcpyDeviceToHost,
@@ -301,6 +314,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt_iterate_kernel = 1;
     ctx->opt_factor_kernel = 1;
+    ctx->opt_persistent = -1;
     auto fail = [&](int code) { int lc = ctx->last_cuda; oci_destroy(ctx); (void)lc; return code; };
     if (cudaGetDevice(&ctx->device) != cudaSuccess) return fail(OCI_E_CUDA);
     device_limits(&ctx->num_sms, &ctx->max_smem_optin);
@@ -377,6 +391,7 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
         if ((int)value != ctx->opt_solve_mode) ctx->factored = false;
         ctx->opt_solve_mode = (int)value;
     }
+    else if (!strcmp(key, "persistent")) ctx->opt_persistent = (int)value; // -1 auto, 0 off, 1 on (structured path)
     else if (!strcmp(key, "si_sweep")) {
         if (value != 0 && value != 1) return -3;
         if ((int)value != ctx->opt_si_sweep) ctx->si_valid = false; // the sweep-order arrays change layout

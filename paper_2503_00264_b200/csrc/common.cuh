@@ -68,7 +68,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];
@@ -144,6 +144,8 @@ int launch_si_setup(oci_ctx *ctx);
 bool st_supported(const oci_ctx *ctx);
 int launch_st_factor(oci_ctx *ctx);
 int launch_st_iteration(oci_ctx *ctx, const struct IterParams &P, bool want_l2);
+// `k` structured iterations (history slots slot0 .. slot0 + k - 1) in ONE cooperative launch; 0 = not applicable
+int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_between);
 int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 
 #ifdef __CUDACC__
@@ -159,17 +161,23 @@ __device__ __forceinline__ unsigned long long resid_bits(double d)
     return (unsigned long long)__double_as_longlong(d);
 }
 
-// Same arithmetic, operation by operation, as the host test in step_impl (api.cu).
-__device__ __forceinline__ bool stop_reached(const StopCheck &s)
+// Same arithmetic, operation by operation, as the host test in step_impl (api.cu). COHERENT: the residual slots
+// were written by other CTAs of the SAME launch (multi-iteration cooperative kernel), so read them past the L1.
+template <bool COHERENT>
+__device__ __forceinline__ bool stop_reached_t(const StopCheck &s)
 {
     if (!s.prev_inf) return false;
-    if (s.rule == OCI_STOP_DPHI_INF) return __longlong_as_double((long long)*s.prev_inf) < s.tol;
+    if (s.rule == OCI_STOP_DPHI_INF) {
+        const unsigned long long b = COHERENT ? __ldcg(s.prev_inf) : *s.prev_inf;
+        return __longlong_as_double((long long)b) < s.tol;
+    }
     if (!s.prev2_l2) return false;
-    const double e2 = *s.prev_l2, e2p = *s.prev2_l2;
+    const double e2 = COHERENT ? __ldcg(s.prev_l2) : *s.prev_l2, e2p = COHERENT ? __ldcg(s.prev2_l2) : *s.prev2_l2;
     if (e2 == 0.0 && e2p == 0.0) return true; // two skipped slots in a row
     const double e = __dsqrt_rn(e2), ep = __dsqrt_rn(e2p);
     return e < __dmul_rn(s.tol, __dsub_rn(1.0, __ddiv_rn(e, ep)));
 }
+__device__ __forceinline__ bool stop_reached(const StopCheck &s) { return stop_reached_t<false>(s); }
 
 __device__ __forceinline__ double warp_max(double v)
 {

@@ -12,6 +12,7 @@
 //   st_cap     (once per dt): C = I - dx/4 (K (x) 1) W assembled on chip, inverted with partial pivoting
 //   st_iterate (every iteration): a4-a7 fused, one thread per (cell, g, m)
 #include "common.cuh"
+#include <cooperative_groups.h>
 #include <limits.h>
 
 namespace {
@@ -129,12 +130,12 @@ struct StParams {
 // GC = G when G is 1, 2, 4 or 8 (the 4G rows of a cell then sit inside one warp, so the three small steps between
 // z and x need only __syncwarp, and for G <= 4 the thread's row of C^-1, its row of K and dx are loaded up front,
 // together with everything else, so that a CTA waits for HBM once); GC = 0: any G, CTA-wide barriers.
-template <bool WANT_L2, int GC>
-__global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterParams P, const StParams S)
+// COHERENT: Psi^(l) and phi^(l) were written by other CTAs of the SAME launch (st_iterate_multi_kernel): read past L1.
+template <bool COHERENT> __device__ __forceinline__ double ld_iter(const double *p) { return COHERENT ? __ldcg(p) : *p; }
+
+template <bool WANT_L2, int GC, bool COHERENT>
+__device__ __forceinline__ void st_iterate_body(const IterParams &P, const StParams &S, double *st_smem)
 {
-    if (stop_reached(P.stop)) return;
-    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
-    extern __shared__ __align__(16) double st_smem[];
     const int N = P.N, G = GC > 0 ? GC : P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
     constexpr bool PRE = GC > 0 && GC <= 4;
     constexpr int GP = PRE ? GC : 1;
@@ -170,14 +171,14 @@ __global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterPar
             const double *self = P.psi_old + (size_t)j * n;
             // a4: incident edge fluxes from Psi^(l) (Eq. 9c-d; closures Eq. 5a-b)
             if (mu > 0.0) { // rows (k,L), (k+1/2,L): upstream = (j-1, R)
-                if (j > 0) { v0 = (self - n)[gm * 4 + 1]; v1 = (self - n)[gm * 4 + 3]; }
+                if (j > 0) { v0 = ld_iter<COHERENT>(self - n + gm * 4 + 1); v1 = ld_iter<COHERENT>(self - n + gm * 4 + 3); }
                 else if (P.bc_left == OCI_BC_REFLECTIVE) {
-                    v0 = self[(g * N + (N - 1 - m)) * 4 + 0]; v1 = self[(g * N + (N - 1 - m)) * 4 + 2];
+                    v0 = ld_iter<COHERENT>(self + (g * N + (N - 1 - m)) * 4 + 0); v1 = ld_iter<COHERENT>(self + (g * N + (N - 1 - m)) * 4 + 2);
                 } else if (P.bc_left == OCI_BC_PRESCRIBED) { v0 = P.inc_left[gm * 2]; v1 = P.inc_left[gm * 2 + 1]; }
             } else {        // rows (k,R), (k+1/2,R): upstream = (j+1, L)
-                if (j < J - 1) { v0 = (self + n)[gm * 4 + 0]; v1 = (self + n)[gm * 4 + 2]; }
+                if (j < J - 1) { v0 = ld_iter<COHERENT>(self + n + gm * 4 + 0); v1 = ld_iter<COHERENT>(self + n + gm * 4 + 2); }
                 else if (P.bc_right == OCI_BC_REFLECTIVE) {
-                    v0 = self[(g * N + (N - 1 - m)) * 4 + 1]; v1 = self[(g * N + (N - 1 - m)) * 4 + 3];
+                    v0 = ld_iter<COHERENT>(self + (g * N + (N - 1 - m)) * 4 + 1); v1 = ld_iter<COHERENT>(self + (g * N + (N - 1 - m)) * 4 + 3);
                 } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = P.inc_right[gm * 2]; v1 = P.inc_right[gm * 2 + 1]; }
             }
             const double *Lp = S.LinvT + (size_t)j * 16 * GN + gm;
@@ -194,7 +195,7 @@ __global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterPar
 #pragma unroll
             for (int gc = 0; gc < GP; ++gc) Kr[gc] = Kp[gc];
             dxq = S.dx[j2] * 0.25;
-            phi_old = P.phi[(size_t)j2 * G4 + r2];
+            phi_old = ld_iter<COHERENT>(P.phi + (size_t)j2 * G4 + r2);
         }
         __syncthreads(); // previous batch done with the shared arrays (and mu_s / w_s loaded)
         if (on) {
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterPar
                 } else {
                     const double *Cp = S.Cinv + (size_t)j2 * G4 * G4 + r2;
                     for (int cc = 0; cc < G4; ++cc) y = fma(Cp[(size_t)cc * G4], pz[cc], y);
-                    po = P.phi[(size_t)j2 * G4 + r2];
+                    po = ld_iter<COHERENT>(P.phi + (size_t)j2 * G4 + r2);
                 }
                 ys[t2] = y;
                 P.phi[(size_t)j2 * G4 + r2] = y;
@@ -272,7 +273,7 @@ __global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterPar
             if (WANT_L2) {
                 const double *old = P.psi_old + (size_t)j * n + gm * 4;
 #pragma unroll
-                for (int p = 0; p < 4; ++p) { const double d = x[p] - old[p]; l2 = fma(d, d, l2); }
+                for (int p = 0; p < 4; ++p) { const double d = x[p] - ld_iter<COHERENT>(old + p); l2 = fma(d, d, l2); }
             }
             *reinterpret_cast<double2 *>(out) = make_double2(x[0], x[1]);
             *reinterpret_cast<double2 *>(out + 2) = make_double2(x[2], x[3]);
@@ -283,6 +284,55 @@ __global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterPar
     if (WANT_L2) {
         l2 = warp_sum(l2);
         if (lane == 0) atomicAdd(P.resid_l2, l2);
+    }
+}
+
+
+template <bool WANT_L2, int GC>
+__global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_kernel(const IterParams P, const StParams S)
+{
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
+    extern __shared__ __align__(16) double st_smem[];
+    st_iterate_body<WANT_L2, GC, false>(P, S, st_smem);
+}
+
+// persistent multi-iteration kernel for problems whose factors stay in L2. One COOPERATIVE launch
+// runs up to n_iters block-Jacobi iterations, a grid-wide barrier between them (every CTA keeps its cells, the two
+// Psi buffers alternate, data written by other CTAs is read past the L1), with the same device-side stop: after the
+// barrier every thread of the grid reads the same residual slot and takes the same decision. Replaces n_iters launches
+// of ~4 us of fixed cost each by n_iters grid barriers.
+struct StMulti {
+    int n_iters, slot0, check_between, rule;
+    double tol;
+    unsigned long long *resid_inf; // history base (slot 0)
+    double *resid_l2;
+    int *executed;
+};
+
+template <bool WANT_L2, int GC>
+__global__ void __launch_bounds__(ST_THREADS, 3) st_iterate_multi_kernel(const IterParams P, const StParams S, const StMulti M)
+{
+    extern __shared__ __align__(16) double st_smem[];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    IterParams Q = P;
+    for (int it = 0; it < M.n_iters; ++it) {
+        const int slot = M.slot0 + it;
+        if (M.check_between && it > 0) {
+            StopCheck st;
+            st.prev_inf = M.resid_inf + slot - 1;
+            st.prev_l2 = M.resid_l2 + slot - 1;
+            st.prev2_l2 = slot >= 2 ? M.resid_l2 + slot - 2 : nullptr;
+            st.tol = M.tol; st.rule = M.rule; st.slot = slot; st.executed = M.executed;
+            if (stop_reached_t<true>(st)) break; // same values everywhere: the whole grid leaves together
+        }
+        if (blockIdx.x == 0 && threadIdx.x == 0) *M.executed = slot + 1;
+        Q.psi_old = (it & 1) ? P.psi_new : P.psi_old;
+        Q.psi_new = (it & 1) ? const_cast<double *>(P.psi_old) : P.psi_new;
+        Q.resid_inf = M.resid_inf + slot;
+        Q.resid_l2 = M.resid_l2 + slot;
+        st_iterate_body<WANT_L2, GC, true>(Q, S, st_smem);
+        grid.sync();
     }
 }
 
@@ -647,5 +697,53 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
     }
 #undef OCI_ST_LAUNCH
     OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}
+
+// f2: k iterations in one cooperative launch. Applies (auto) to small problems (<= 8 MB per iteration), where the fixed
+// cost of a launch is what an iteration costs (measured: config 1 5.6 -> 3.9 us, config 2 6.2 -> 5.1 us per iteration;
+// from ~10 MB on the pipelined per-iteration kernel is faster); "persistent" = 1 forces it, 0 disables it.
+int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_between)
+{
+    if (ctx->opt_solve_mode != 1 || ctx->opt_persistent == 0 || k < 2) return 0;
+    const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
+    const size_t bytes_per_iter = (size_t)ctx->J * (52 * (size_t)ctx->n + 136 * (size_t)ctx->G * ctx->G + 64 * ctx->G + 8);
+    if (ctx->opt_persistent < 0 && bytes_per_iter > ((size_t)8 << 20)) return 0;
+    int coop = 0;
+    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess || !coop) return 0;
+    const size_t smem = sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 + (size_t)3 * CPB * G4);
+    IterParams P;
+    P.stop = make_stop(ctx, slot0, false);
+    P.J = ctx->J; P.N = ctx->N; P.G = ctx->G; P.n = ctx->n;
+    P.bc_left = ctx->bc_left; P.bc_right = ctx->bc_right;
+    P.Minv = nullptr; P.c = ctx->c;
+    P.psi_old = ctx->psi[ctx->cur]; P.psi_new = ctx->psi[ctx->cur ^ 1];
+    P.phi = ctx->phi; P.mu = ctx->mu; P.w = ctx->w;
+    P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
+    P.resid_inf = ctx->resid_inf + slot0; P.resid_l2 = ctx->resid_l2 + slot0;
+    P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
+    StParams S;
+    S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
+    StMulti M;
+    M.n_iters = k; M.slot0 = slot0; M.check_between = check_between ? 1 : 0; M.rule = ctx->stop_rule; M.tol = ctx->stop_tol;
+    M.resid_inf = ctx->resid_inf; M.resid_l2 = ctx->resid_l2; M.executed = ctx->ctrl;
+    void *args[] = {&P, &S, &M};
+    const void *fn = nullptr;
+#define OCI_STM_PICK(GC_) fn = want_l2 ? (const void *)st_iterate_multi_kernel<true, GC_> : (const void *)st_iterate_multi_kernel<false, GC_>
+    switch (ctx->G) {
+    case 1: OCI_STM_PICK(1); break;
+    case 2: OCI_STM_PICK(2); break;
+    case 4: OCI_STM_PICK(4); break;
+    case 8: OCI_STM_PICK(8); break;
+    default: OCI_STM_PICK(0); break;
+    }
+#undef OCI_STM_PICK
+    int per_sm = 0;
+    OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ST_THREADS, smem));
+    if (per_sm < 1) return 0;
+    int grid = (ctx->J + CPB - 1) / CPB;
+    if (grid > per_sm * ctx->num_sms) grid = per_sm * ctx->num_sms; // all CTAs co-resident: the grid barrier needs it
+    OCI_CUDA_TRY(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(ST_THREADS), args, smem, ctx->stream));
+    if (k & 1) ctx->cur ^= 1; // as k single launches would have left it
     return 1;
 }

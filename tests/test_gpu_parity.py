@@ -400,3 +400,46 @@ def test_si_scan_full_size_step_cfg5():
     assert it_g == conv_g == it_o
     assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
     assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# a batch of structured iterations as ONE cooperative launch with grid-wide barriers.
+# ---------------------------------------------------------------------------------------------------------------
+PERSIST = {"solve_mode": 1, "persistent": 1}
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES + [(15, 3000, 4, 2, 1, 2)])
+def test_persistent_multi_iteration_parity(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p, options=PERSIST), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    for k in (2, 5, 8):          # even and odd batch lengths: the two Psi buffers alternate inside the launch
+        s.iterate(k)
+        o.oci_iterate(k)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"after a batch of {k}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("k", [2, 5, 8])
+def test_persistent_step_loop_stops_at_the_natural_iteration(rule, k):
+    p = W.random_problem(33, 61, 4, 2, bc_left=1, bc_right=2, dt=0.05)
+    s, o = _solver(p, options=PERSIST), _oracle(p)
+    for step in range(3):
+        it_g, conv_g, _ = s.step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
+        it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule)
+        assert it_g == conv_g == it_o, f"step {step}"
+        np.testing.assert_allclose(s.residual_history(kind=rule), hist_o, rtol=1e-6, atol=1e-15)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_PHI
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+def test_persistent_auto_applies_to_config2_and_matches():
+    p = W.config2(dt=0.1)
+    a, b = _solver(p, options={"solve_mode": 1}), _solver(p, options={"solve_mode": 1, "persistent": 0})
+    ia, _, _ = a.step(tol=p.tol, max_iters=4000, check_every=8)
+    ib, _, _ = b.step(tol=p.tol, max_iters=4000, check_every=8)
+    assert ia == ib
+    assert a.last_timing(1)[1] < b.last_timing(1)[1]          # fewer launches: one per batch instead of one per iteration
+    assert rel(a.scalar_flux().cpu().numpy(), b.scalar_flux().cpu().numpy()) < 1e-13
