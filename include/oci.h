@@ -119,9 +119,11 @@ int oci_factor(oci_ctx *ctx);
  * Psi_j^(l+1) = A_j^{-1} b_j, phi^(l+1), residual. Builds the constant part c_j first if it is stale. [async] */
 int oci_iterate(oci_ctx *ctx, int32_t n_iters);
 
-/* One whole time step (Alg. 2): const RHS, iterate until the stop rule holds (tested on the host from a
- * device-side residual read once every check_every iterations, so up to check_every-1 extra iterations may
- * run), then advance psi_{k+1/2} -> psi_{k-1/2} (a8) if advance != 0.
+/* One whole time step (Alg. 2): a1 + a2 if the factors are stale, const RHS, iterate until the stop rule holds, then
+ * advance psi_{k+1/2} -> psi_{k-1/2} (a8) if advance != 0. Iterations are enqueued check_every at a time; every
+ * iteration after the first of a batch looks at the residual of the one before it ON THE DEVICE and skips itself
+ * once the rule held, so exactly the natural number of iterations runs; the host reads the residuals and the
+ * executed-iterations counter once per batch (the only host round-trip).
  * iters_out[0] = iterations performed, iters_out[1] = iterations after which the rule first held (0 if never);
  * resid_out = last tested residual. Either may be NULL. [sync] */
 int oci_step(oci_ctx *ctx, double tol, int32_t max_iters, int32_t check_every, int32_t stop_rule,
