@@ -61,6 +61,9 @@ def lib():
         L.orc_oci_converge.argtypes = [_i, _i, _i, _dp, _dp, _i, _i, _dp, _dp, _dp, _ip, _dp, _d, _i, _i, _dp,
                                        _dp, _dp, _dp]
         L.orc_oci_converge.restype = _i
+        L.orc_oci_iterate_redblack.argtypes = [_i, _i, _i, _dp, _i, _i, _dp, _dp, _dp, _ip, _dp, _dp]
+        L.orc_oci_converge_redblack.argtypes = L.orc_oci_converge.argtypes
+        L.orc_oci_converge_redblack.restype = _i
         L.orc_si_converge.argtypes = [_i, _i, _i, _dp, _dp, _dp, _dp, _dp, _dp, _d, _i, _i, _dp, _dp, _dp, _dp,
                                       _d, _i, _i, _dp, _dp, _dp, _dp]
         L.orc_si_converge.restype = _i
@@ -149,10 +152,18 @@ class Oracle:
         lib().orc_scalar_flux(self.J, self.N, self.G, self.w, np.ascontiguousarray(psi), phi)
         return phi
 
-    def oci_iterate(self, n_iters: int = 1):
-        """n_iters block-Jacobi iterations on the current iterate (requires factor() and const_rhs())."""
+    def oci_iterate(self, n_iters: int = 1, ordering: int = 0):
+        """n_iters block-Jacobi (ordering 0, the paper's OCI) or red-black (ordering 1) iterations
+        on the current iterate (requires factor() and const_rhs())."""
         if self.LU is None:
             raise RuntimeError("factor() first")
+        if ordering == 1:
+            self.psi = np.ascontiguousarray(self.psi).copy()
+            for _ in range(n_iters):
+                lib().orc_oci_iterate_redblack(self.J, self.N, self.G, self.mu, self.bc_left, self.bc_right,
+                                               self.inc_left, self.inc_right, self.LU, self.piv, self.c, self.psi)
+            self.phi = self.scalar_flux(self.psi)
+            return self.psi
         for _ in range(n_iters):
             new = np.empty_like(self.psi)
             lib().orc_oci_iterate(self.J, self.N, self.G, self.mu, self.bc_left, self.bc_right, self.inc_left,
@@ -174,16 +185,18 @@ class Oracle:
     def _advance(self):
         self.psi_prev = np.ascontiguousarray(self.psi[..., 2:4]).copy()
 
-    def oci_step(self, tol: float = 1e-8, max_iters: int = 100000, rule: int = 0, advance: bool = True):
+    def oci_step(self, tol: float = 1e-8, max_iters: int = 100000, rule: int = 0, advance: bool = True,
+                 ordering: int = 0):
         """Converge one time step with OCI; returns (iterations, residual history)."""
         if self.LU is None:
             self.factor()
         self.const_rhs()
         work = np.empty(self.J * self.n)
         resid = np.zeros(max_iters)
-        it = lib().orc_oci_converge(self.J, self.N, self.G, self.mu, self.w, self.bc_left, self.bc_right,
-                                    self.inc_left, self.inc_right, self.LU, self.piv, self.c, tol, max_iters, rule,
-                                    self.psi.reshape(-1), self.phi.reshape(-1), work, resid)
+        fn = lib().orc_oci_converge_redblack if ordering == 1 else lib().orc_oci_converge
+        self.psi = np.ascontiguousarray(self.psi)
+        it = fn(self.J, self.N, self.G, self.mu, self.w, self.bc_left, self.bc_right, self.inc_left, self.inc_right,
+                self.LU, self.piv, self.c, tol, max_iters, rule, self.psi.reshape(-1), self.phi.reshape(-1), work, resid)
         if advance:
             self._advance()
         return it, resid[:it].copy()

@@ -85,3 +85,46 @@ def test_rule1_controls_false_convergence():
     assert err1 < err0
     if exact is not None:
         assert np.abs(ref.psi - exact).max() < 1e-11
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Red-black ordering of the cell solves: pins of oracle.oci_iterate(ordering=1)
+# ---------------------------------------------------------------------------------------------------------------
+def test_one_redblack_iteration_is_block_gauss_seidel_of_the_global_system():
+    """Even cells from the old iterate, then odd cells from the new even cells: two half-steps on the global matrix,
+    done here with numpy on the independently assembled global system."""
+    from pins import global_system
+    p = W.random_problem(22, J=7, N=4, G=2, bc_left=W.BC_REFLECTIVE, bc_right=W.BC_PRESCRIBED)
+    M, rhs = global_system(p, p.q, p.psi0)
+    n = p.n
+    o = oracle.Oracle(p)
+    D = np.zeros_like(M)
+    for j in range(p.J):
+        D[j * n:(j + 1) * n, j * n:(j + 1) * n] = o.assemble_cell(j)   # the lagged reflective term is NOT in A_0 (A12)
+    Off = M - D
+    rng = np.random.default_rng(1)
+    x = rng.uniform(0, 1, size=M.shape[0])
+    want = x.copy()
+    for colour in (0, 1):
+        r = rhs - Off @ want
+        for j in range(colour, p.J, 2):
+            want[j * n:(j + 1) * n] = np.linalg.solve(D[j * n:(j + 1) * n, j * n:(j + 1) * n], r[j * n:(j + 1) * n])
+    o.set_iterate(x)
+    o.factor()
+    o.const_rhs()
+    got = o.oci_iterate(1, ordering=1).reshape(-1)
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-13 * np.abs(want).max())
+
+
+def test_redblack_reaches_the_same_fixed_point_in_about_half_the_iterations():
+    """Same fixed point as the global solve; for this consistently ordered block-tridiagonal system the Gauss-Seidel
+    rate is the square of the Jacobi rate, so about half the iterations."""
+    p = W.config2(dt=1.0, J=96)       # thin cells, c = 0.9: slow convergence, several hundred Jacobi iterations
+    exact = global_solve(p, p.q, p.psi0)
+    jac, rb = oracle.Oracle(p), oracle.Oracle(p)
+    it_j, _ = jac.oci_step(tol=1e-12, max_iters=20000, rule=0, advance=False)
+    it_r, hist = rb.oci_step(tol=1e-12, max_iters=20000, rule=0, advance=False, ordering=1)
+    scale = max(np.abs(exact).max(), 1e-300)
+    np.testing.assert_allclose(rb.psi, exact, rtol=0, atol=1e-10 * scale + 1e-12)
+    np.testing.assert_allclose(jac.psi, exact, rtol=0, atol=1e-10 * scale + 1e-12)
+    assert 0.4 * it_j <= it_r <= 0.65 * it_j, (it_j, it_r)
