@@ -97,7 +97,11 @@ int oci_last_cuda_error(const oci_ctx *ctx);
  * the comparator north_star names; 1 = the same sweep evaluated as a parallel scan of the per-cell affine edge maps,
  * same iterates to rounding), "persistent" (structured path only: -1 [default] = run a batch
  * of iterations as ONE cooperative launch with grid-wide barriers when the problem is small (<= 8 MB per iteration),
- * 0 = never, 1 = always). Returns -2 for an unknown key, -3 for a bad value. */
+ * 0 = never, 1 = always), "ordering" (structured path only: 0 = block-Jacobi [default], the
+ * paper's OCI; 1 = red-black: per iteration the even cells, then the odd cells from the new even ones, in place --
+ * the block Gauss-Seidel variant PAPER.md:29, 550 names, about half the iterations; SURVEY.md 8(f) row f4;
+ * oci_iterate / oci_step return OCI_E_UNSUPPORTED in the dense mode). Returns -2 for an unknown key, -3 for a bad
+ * value. */
 int oci_set_option(oci_ctx *ctx, const char *key, int64_t value);
 
 int oci_set_dt(oci_ctx *ctx, double dt);                               /* invalidates the factors      */

@@ -250,7 +250,8 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
         }
         const int executed = *h_exec; // iterations of this step that really ran (<= it + k)
         if (executed < it + 1 || executed > it + k) return OCI_E_STATE;
-        if (scheme == 0 && ((it + k - executed) & 1)) ctx->cur ^= 1; // skipped launches did not swap the Jacobi buffers
+        // skipped launches did not swap the Jacobi buffers (red-black works in place: nothing to undo)
+        if (scheme == 0 && ctx->opt_ordering == 0 && ((it + k - executed) & 1)) ctx->cur ^= 1;
         const int l = executed - 1;
         last = want_l2 ? sqrt(h_l2[l]) : h_inf[l];
         if (executed < it + k) conv_at = executed;                       // the device saw the rule hold at slot l
@@ -390,6 +391,10 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
         if (value == 1 && !st_supported(ctx)) return OCI_E_UNSUPPORTED;
         if ((int)value != ctx->opt_solve_mode) ctx->factored = false;
         ctx->opt_solve_mode = (int)value;
+    }
+    else if (!strcmp(key, "ordering")) {
+        if (value != 0 && value != 1) return -3;
+        ctx->opt_ordering = (int)value;
     }
     else if (!strcmp(key, "persistent")) ctx->opt_persistent = (int)value; // -1 auto, 0 off, 1 on (structured path)
     else if (!strcmp(key, "si_sweep")) {

@@ -68,7 +68,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];
@@ -120,6 +120,7 @@ struct IterParams {
     int n_items;
     int stages;   // matrix ring depth
     int chunk_doubles;
+    int color, ncolors;   // structured path: cells j = ncolors * i + color (ncolors = 1: all cells)
 };
 
 static inline ProblemView make_view(const oci_ctx *c)

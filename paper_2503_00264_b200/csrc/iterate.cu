@@ -581,6 +581,8 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
     P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
     P.resid_inf = ctx->resid_inf + hist_slot;
     P.resid_l2 = ctx->resid_l2 + hist_slot;
+    P.color = 0; P.ncolors = 1;
+    if (ctx->opt_ordering == 1 && ctx->opt_solve_mode != 1) return OCI_E_UNSUPPORTED; // red-black: structured path only
     const bool wpc_ok = ctx->n == 64 || ctx->n == 128 || ctx->n == 256;
     if (ctx->opt_solve_mode == 1) {
         P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
@@ -639,6 +641,7 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
         else oci_iterate_stream_kernel<false><<<pl.grid, ITER_THREADS, pl.smem, ctx->stream>>>(P);
     }
     OCI_CUDA_TRY(ctx, cudaGetLastError());
+    if (ctx->opt_ordering == 1) return 2; // red-black updates the current iterate in place: no buffer swap
     ctx->cur ^= 1;
     return 1;
 }

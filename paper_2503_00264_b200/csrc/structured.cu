@@ -158,9 +158,11 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
         else __syncthreads();
     };
 
-    for (int base = blockIdx.x * CPB; base < J; base += gridDim.x * CPB) {
-        const int j = base + a;
-        const bool on = lane_on && j < J;
+    // ordering: all cells (ncolors = 1, Jacobi) or the cells of one colour (ncolors = 2: j = 2 i + color), in place
+    const int NC = P.ncolors, Jc = (J - P.color + NC - 1) / NC;
+    for (int base = blockIdx.x * CPB; base < Jc; base += gridDim.x * CPB) {
+        const int j = NC * (base + a) + P.color;
+        const bool on = lane_on && base + a < Jc;
         double L[16], z[4], b[4], v0 = 0.0, v1 = 0.0, mu = 1.0;
         // ---- all global loads of this batch up front
         if (on) {
@@ -186,8 +188,8 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
             for (int k = 0; k < 16; ++k) L[k] = Lp[(size_t)k * GN];
         }
         double Cr[4 * GP], Kr[GP], dxq = 0.0, phi_old = 0.0; // this thread's (first) row of the 4G-system
-        if (PRE && tid < rows && base + tid / G4 < J) {
-            const int a2 = tid / G4, r2 = tid - a2 * G4, j2 = base + a2;
+        if (PRE && tid < rows && base + tid / G4 < Jc) {
+            const int a2 = tid / G4, r2 = tid - a2 * G4, j2 = NC * (base + a2) + P.color;
             const double *Cp = S.Cinv + (size_t)j2 * G4 * G4 + r2;
 #pragma unroll
             for (int cc = 0; cc < 4 * GP; ++cc) Cr[cc] = Cp[(size_t)cc * G4];
@@ -213,7 +215,7 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
         // thread-iteration (4G rows per cell; 4G > G N when N = 2, hence the loops)
         for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
             const int a2 = t2 / G4, r2 = t2 - a2 * G4;
-            if (base + a2 < J) {
+            if (base + a2 < Jc) {
                 const int g2 = r2 >> 2, p2 = r2 & 3;
                 const double *src = wz + ((size_t)a2 * GN + g2 * N) * 4 + p2;
                 double acc = 0.0;
@@ -223,8 +225,8 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
         }
         small_sync();
         for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
-            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = base + a2;
-            if (j2 < J) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = NC * (base + a2) + P.color;
+            if (base + a2 < Jc) {
                 const double *pz = phiz + a2 * G4;
                 double y = 0.0, po;
                 if (PRE && t2 == tid) {
@@ -244,8 +246,8 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
         }
         small_sync();
         for (int t2 = tid; t2 < rows; t2 += ST_THREADS) {
-            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = base + a2;
-            if (j2 < J) {
+            const int a2 = t2 / G4, r2 = t2 - a2 * G4, j2 = NC * (base + a2) + P.color;
+            if (base + a2 < Jc) {
                 const int g2 = r2 >> 2, p2 = r2 & 3;
                 const double *yy = ys + a2 * G4 + p2;
                 double acc = 0.0;
@@ -623,7 +625,8 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
     StParams S;
     S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
     const int GN = ctx->G * ctx->N, G4 = 4 * ctx->G;
-    if (ctx->opt_iterate_kernel == 1) { // persistent bulk-copy pipeline; falls through when the ring would not fit
+    if (ctx->opt_iterate_kernel == 1 && ctx->opt_ordering == 0) { // persistent bulk-copy pipeline (Jacobi ordering);
+                                                                  // falls through when the ring would not fit
         // 256 consumer threads and two CTAs per SM; 128 and four when a cell takes a whole warp (measured: config 3,
         // G N = 32, 16.5 -> 13.4 us per iteration; config 5, G N = 16, is faster with 256: 45 against 47 us)
         const int CT = (GN > 16 && GN <= 32 && ctx->opt_ctas_per_sm != 2) ? 128 : 256, CPB = CT / GN;
@@ -682,22 +685,32 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
     }
     const int CPB = ST_THREADS / GN;
     const size_t smem = sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 + (size_t)3 * CPB * G4);
-    const int grid = (ctx->J + CPB - 1) / CPB; // one batch of CPB cells per CTA: CTA turnover hides the load latency
 #define OCI_ST_LAUNCH(GC_)                                                                                         \
     do {                                                                                                           \
-        if (want_l2) st_iterate_kernel<true, GC_><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);                  \
-        else st_iterate_kernel<false, GC_><<<grid, ST_THREADS, smem, ctx->stream>>>(P, S);                         \
+        if (want_l2) st_iterate_kernel<true, GC_><<<grid, ST_THREADS, smem, ctx->stream>>>(Q, S);                  \
+        else st_iterate_kernel<false, GC_><<<grid, ST_THREADS, smem, ctx->stream>>>(Q, S);                         \
     } while (0)
-    switch (ctx->G) {
-    case 1: OCI_ST_LAUNCH(1); break;
-    case 2: OCI_ST_LAUNCH(2); break;
-    case 4: OCI_ST_LAUNCH(4); break;
-    case 8: OCI_ST_LAUNCH(8); break;
-    default: OCI_ST_LAUNCH(0); break;
+    // ordering 1 (red-black): the even cells, then the odd cells, in place on the current iterate
+    const int ncolors = ctx->opt_ordering == 1 ? 2 : 1;
+    for (int color = 0; color < ncolors; ++color) {
+        IterParams Q = P;
+        Q.color = color;
+        Q.ncolors = ncolors;
+        if (ncolors == 2) Q.psi_new = const_cast<double *>(P.psi_old);
+        const int Jc = (ctx->J - color + ncolors - 1) / ncolors;
+        if (Jc < 1) continue;
+        const int grid = (Jc + CPB - 1) / CPB; // one batch of CPB cells per CTA: CTA turnover hides the load latency
+        switch (ctx->G) {
+        case 1: OCI_ST_LAUNCH(1); break;
+        case 2: OCI_ST_LAUNCH(2); break;
+        case 4: OCI_ST_LAUNCH(4); break;
+        case 8: OCI_ST_LAUNCH(8); break;
+        default: OCI_ST_LAUNCH(0); break;
+        }
     }
 #undef OCI_ST_LAUNCH
     OCI_CUDA_TRY(ctx, cudaGetLastError());
-    return 1;
+    return ncolors;
 }
 
 // f2: k iterations in one cooperative launch. Applies (auto) to small problems (<= 8 MB per iteration), where the fixed
@@ -705,7 +718,7 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
 // from ~10 MB on the pipelined per-iteration kernel is faster); "persistent" = 1 forces it, 0 disables it.
 int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_between)
 {
-    if (ctx->opt_solve_mode != 1 || ctx->opt_persistent == 0 || k < 2) return 0;
+    if (ctx->opt_solve_mode != 1 || ctx->opt_persistent == 0 || ctx->opt_ordering != 0 || k < 2) return 0;
     const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
     const size_t bytes_per_iter = (size_t)ctx->J * (52 * (size_t)ctx->n + 136 * (size_t)ctx->G * ctx->G + 64 * ctx->G + 8);
     if (ctx->opt_persistent < 0 && bytes_per_iter > ((size_t)8 << 20)) return 0;
@@ -722,6 +735,7 @@ int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_bet
     P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
     P.resid_inf = ctx->resid_inf + slot0; P.resid_l2 = ctx->resid_l2 + slot0;
     P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
+    P.color = 0; P.ncolors = 1;
     StParams S;
     S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
     StMulti M;

@@ -443,3 +443,59 @@ def test_persistent_auto_applies_to_config2_and_matches():
     assert ia == ib
     assert a.last_timing(1)[1] < b.last_timing(1)[1]          # fewer launches: one per batch instead of one per iteration
     assert rel(a.scalar_flux().cpu().numpy(), b.scalar_flux().cpu().numpy()) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# SURVEY 8(f) row f4 (first half): red-black ordering of the cell solves ("ordering" = 1, structured path).
+# ---------------------------------------------------------------------------------------------------------------
+RB = {"solve_mode": 1, "ordering": 1}
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES + [(16, 1001, 8, 2, 1, 2)])
+def test_redblack_per_iteration_parity(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p, options=RB), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    for l in range(5):
+        s.iterate(1)
+        o.oci_iterate(1, ordering=1)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"iteration {l + 1}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+    s.iterate(6)
+    o.oci_iterate(6, ordering=1)
+    assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("k", [1, 5])
+def test_redblack_step_loop_matches_oracle(rule, k):
+    p = W.random_problem(33, 61, 4, 2, bc_left=1, bc_right=2, dt=0.05)
+    s, o = _solver(p, options=RB), _oracle(p)
+    for step in range(3):
+        it_g, conv_g, _ = s.step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
+        it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule, ordering=1)
+        assert it_g == conv_g == it_o, f"step {step}"
+        np.testing.assert_allclose(s.residual_history(kind=rule), hist_o, rtol=1e-6, atol=1e-15)
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+def test_redblack_config5_full_size_halves_the_iterations():
+    p = W.config5(dt=1.0)
+    rb, jac, o = _solver(p, options=RB), _solver(p, options={"solve_mode": 1}), _oracle(p)
+    it_r, conv_r, _ = rb.step(tol=p.tol, max_iters=4000, check_every=8)
+    it_j, _, _ = jac.step(tol=p.tol, max_iters=4000, check_every=8)
+    it_o, _ = o.oci_step(tol=p.tol, max_iters=4000, ordering=1)
+    assert it_r == conv_r == it_o
+    assert it_r < 0.65 * it_j
+    assert rel(rb.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
+    assert float((rb.scalar_flux() - jac.scalar_flux()).abs().max()) < 1e-6     # both stopped at tol 1e-8
+
+
+def test_redblack_needs_the_structured_path():
+    p = W.random_problem(2, 9, 4, 1)
+    s = _solver(p, options={"ordering": 1})
+    s.factor()
+    with pytest.raises(Exception):
+        s.iterate(1)
