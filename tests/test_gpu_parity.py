@@ -451,7 +451,7 @@ def test_persistent_auto_applies_to_config2_and_matches():
 RB = {"solve_mode": 1, "ordering": 1}
 
 
-@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES + [(16, 1001, 8, 2, 1, 2)])
+@pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES + [(16, 1001, 8, 2, 1, 2), (17, 1000, 16, 1, 0, 1)])
 def test_redblack_per_iteration_parity(seed, J, N, G, bl, br):
     p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
     s, o = _solver(p, options=RB), _oracle(p)
