@@ -158,6 +158,11 @@ int oci_step_host(oci_ctx *ctx, int32_t scheme, const double *q_host, double tol
 
 /* Debug / parity helpers (tests only). A_host, Ainv_host: [n][n] row-major. [sync] */
 int oci_debug_get_matrix(oci_ctx *ctx, int32_t cell, double *A_host);   /* assembled, un-eliminated A_j  */
+/* The same matrix as the PRODUCTION factor kernel selected by the current options assembles it on chip (a1 inside the
+ * a1 + a2 launch), dumped before the elimination starts -- what the bit-exactness test of the production assembly
+ * reads. OCI_E_UNSUPPORTED when that kernel assembles through the same device function as oci_debug_get_matrix
+ * (the generic shared-memory kernel) or in solve_mode 1. */
+int oci_debug_get_factor_input(oci_ctx *ctx, int32_t cell, double *A_host);
 int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host);/* what oci_factor stored for j
                                                                           (OCI_E_UNSUPPORTED in solve_mode 1) */
 int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev);               /* [J][n] c_j of a3 [async]       */

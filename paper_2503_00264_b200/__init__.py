@@ -58,6 +58,7 @@ _SIGNATURES = {
                                 _dptr]),
     "oci_debug_get_matrix": (C.c_int, [_dptr, _i32, _dptr]),
     "oci_debug_get_inverse": (C.c_int, [_dptr, _i32, _dptr]),
+    "oci_debug_get_factor_input": (C.c_int, [_dptr, _i32, _dptr]),
     "oci_debug_get_const_rhs": (C.c_int, [_dptr, _dptr]),
     "oci_last_timing": (C.c_int, [_dptr, _i32, C.POINTER(_f64), C.POINTER(_i64)]),
 }
@@ -259,6 +260,13 @@ class OCISolver:
     def debug_matrix(self, cell: int):
         out = self._np.empty((self.n, self.n))
         self._check("oci_debug_get_matrix", self.lib.oci_debug_get_matrix(self._ctx, int(cell), out.ctypes.data))
+        return out
+
+    def debug_factor_input(self, cell: int):
+        """The tile the production factor kernel assembles on chip for `cell`, dumped before the elimination."""
+        out = self._np.empty((self.n, self.n))
+        self._check("oci_debug_get_factor_input",
+                    self.lib.oci_debug_get_factor_input(self._ctx, int(cell), out.ctypes.data))
         return out
 
     def debug_inverse(self, cell: int):

@@ -315,6 +315,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt_iterate_kernel = 1;
     ctx->opt_factor_kernel = 1;
+    ctx->opt_factor_update = 1;
     ctx->opt_persistent = -1;
     auto fail = [&](int code) { int lc = ctx->last_cuda; oci_destroy(ctx); (void)lc; return code; };
     if (cudaGetDevice(&ctx->device) != cudaSuccess) return fail(OCI_E_CUDA);
@@ -384,7 +385,8 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     if (!strcmp(key, "iterate_kernel")) ctx->opt_iterate_kernel = (int)value;
     else if (!strcmp(key, "iterate_stages")) ctx->opt_stages = (int)value;
     else if (!strcmp(key, "iterate_ctas_per_sm")) ctx->opt_ctas_per_sm = (int)value;
-    else if (!strcmp(key, "factor_kernel")) ctx->opt_factor_kernel = (int)value;
+    else if (!strcmp(key, "factor_kernel")) { ctx->opt_factor_kernel = (int)value; ctx->factored = false; }
+    else if (!strcmp(key, "factor_update")) { ctx->opt_factor_update = (int)value; ctx->factored = false; }
     else if (!strcmp(key, "refactor_every_step")) ctx->opt_refactor_every_step = (int)value;
     else if (!strcmp(key, "solve_mode")) {
         if (value != 0 && value != 1) return -3;
@@ -578,6 +580,20 @@ int oci_debug_get_matrix(oci_ctx *ctx, int32_t cell, double *A_host)
     if (!A_host) return -3;
     int r = launch_assemble_one(ctx, cell, ctx->scratch);
     if (r < 0) return r;
+    OCI_CUDA_TRY(ctx, cudaMemcpyAsync(A_host, ctx->scratch, sizeof(double) * (size_t)ctx->n * ctx->n,
+                                      cudaMemcpyDeviceToHost, ctx->stream));
+    OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    return 0;
+}
+
+int oci_debug_get_factor_input(oci_ctx *ctx, int32_t cell, double *A_host)
+{
+    if (!ctx) return -1;
+    if (cell < 0 || cell >= ctx->J) return -2;
+    if (!A_host) return -3;
+    int r = launch_factor_input(ctx, cell, ctx->scratch);
+    if (r < 0) return r;
+    if (r == 0) return OCI_E_UNSUPPORTED;
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(A_host, ctx->scratch, sizeof(double) * (size_t)ctx->n * ctx->n,
                                       cudaMemcpyDeviceToHost, ctx->stream));
     OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));

@@ -68,7 +68,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering;
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];
@@ -135,6 +135,7 @@ static inline ProblemView make_view(const oci_ctx *c)
 // launchers implemented in the kernel translation units (each returns the number of kernels launched, < 0 on error)
 int launch_factor(oci_ctx *ctx);
 int launch_assemble_one(oci_ctx *ctx, int cell, double *A_dev_rowmajor);
+int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor);
 int launch_const_rhs(oci_ctx *ctx);
 int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 StopCheck make_stop(const oci_ctx *ctx, int slot, bool check_prev);

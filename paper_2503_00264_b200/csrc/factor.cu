@@ -637,6 +637,512 @@ __global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restr
     }
 }
 
+// ============================================================================================================
+// n = 64: ONE WARP PER CELL, the working matrix in shared memory, rank-8 updates on the FP64 tensor path (DMMA):
+// the production a1 + a2 kernel of the headline configuration.
+// ============================================================================================================
+// Partial pivoting makes the 64 pivot decisions of a cell strictly sequential, and each is a chain of dependent
+// latencies (arg-max reduction, ballot, broadcast of the pivot row, one fused multiply-add). The throughput of the
+// kernel is therefore (cells in flight per SM) / (length of that chain), and the chain is shortest when NOTHING in it
+// crosses a warp: no CTA barrier, no exchange through another warp. So a cell belongs to one warp from assembly to
+// store, six cells (warps) are resident per SM and drift apart in phase, which overlaps one cell's pivot chain with
+// another cell's rank-8 update.
+//   W      column-major in shared memory, leading dimension 66: lane l reads rows {2 l, 2 l + 1} of a column as one
+//          conflict-free 16-byte access (assembly, panel phase, store), and the 8 x 8 accumulator fragments of
+//          mma.sync.m8n8k4.f64 (lane holds row l / 4, columns 2 (l % 4), + 1) are conflict-free 8-byte accesses
+//          (66 = 2 mod 8 spreads the four columns of a half-warp over all 32 banks).
+//   phase P (panel of 8 columns, in registers, two rows per lane): per pivot step the local winner of the lane's two
+//          rows (exact 64-bit compare, lower row on a tie), redux.sync.max on the high key word + ballot (exact tie
+//          path behind a warp-uniform branch: first maximal |entry|), every lane scales its candidate row by a
+//          branch-free reciprocal in the shadow of the reduction, the winner broadcasts its scaled row through 64
+//          bytes of shared memory, 16 fused multiply-adds per lane.
+//   phase U  W[:, c] += Z W_old[R, c] for the 56 other columns, Z = T[:, R] - I[:, R]: per 8 x 8 tile two
+//          mma.sync.m8n8k4.f64 with the A fragments (Z, read from the eliminated panel in place) and the B fragments
+//          (the 8 pivot rows of the column block, read before the block is touched) held in registers. A DMMA carries
+//          8 fused multiply-adds per lane in ONE issue slot at the full rate of the FP64 pipe (measured on this B200:
+//          16.5 cycles per DMMA and sub-partition = 64 FMA/clk/SM from one warp per sub-partition; the DFMA form of
+//          the same update needs 8 issue slots and 4.5 shared-memory loads per 8 FMAs) -- DMMA_UPD = false keeps that
+//          form for the A/B measurement DESIGN.md quotes.
+//   store  rows and columns un-scrambled on the way out: lane l gathers rows {rho[2 l], rho[2 l + 1]} of column
+//          rhoinv[c] and writes 16 contiguous bytes of column c of A^{-1}.
+// Cells are handed out by an atomic counter (a static split would leave the sub-partitions that hold two of the six
+// warps behind).
+constexpr int WC_LD = 66;
+
+struct WcShared {
+    double W[64 * WC_LD];          // [column][row], column-major working matrix
+    double prow[2][FR_NB];         // [step parity][c]: the scaled pivot row of the current step
+    int rho[64], rhoinv[64];
+};
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c0), "+d"(c1)
+        : "d"(a), "d"(b));
+}
+
+// a1 for one warp: rows {2 lane, 2 lane + 1} of every column of A_j into the column-major shared-memory array W
+// (leading dimension ld). Same operations in the same order as a_entry(): bit-identical (asserted by
+// tests/test_gpu_parity.py::test_production_assembly_bit_exact through oci_debug_get_factor_input).
+__device__ __forceinline__ void assemble_rows2(const ProblemView &P, int cell, int lane, double *W, int ld,
+                                               int bmc0 = 0, int bmc_step = 1)
+{
+    const int N = P.N, G = P.G, NB = N * G;
+    const double dx = P.dx[cell];
+    for (int rb = 0; rb < P.n; rb += 64) { // row block: rows rb + 2 lane, + 1
+        const int p0 = (lane & 1) * 2;
+        const int bm = (rb >> 2) + (lane >> 1), m = bm % N, g = bm / N;
+        const double sig = P.sigma_t[(size_t)cell * G + g], mu = P.mu[m];
+        const double av = __dmul_rn(__dadd_rn(fabs(mu), __dmul_rn(dx, sig)), 0.5);
+        const double gam = __ddiv_rn(dx, __dmul_rn(P.v[g], P.dt));
+        const double h = __dmul_rn(mu, 0.5), hg = __dmul_rn(gam, 0.5), ga = __dadd_rn(gam, av);
+        const double *Krow = P.transfer + ((size_t)cell * G + g) * G;
+        for (int bmc = bmc0; bmc < NB; bmc += bmc_step) { // column block (g', m')
+            const double Kw = __dmul_rn(__dmul_rn(__dmul_rn(dx, Krow[bmc / N]), 0.25), P.w[bmc % N]);
+            const bool diag = bm == bmc;
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp) {
+                double val[2];
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int p = p0 + e, d = pp - p;
+                    double x = 0.0;
+                    if (diag) { // Eq. 8b
+                        if (d == 0) x = p < 2 ? av : ga;
+                        else if (p == 0 && pp == 1) x = h;
+                        else if (p == 1 && pp == 0) x = -h;
+                        else if (p == 2 && pp == 3) x = h;
+                        else if (p == 3 && pp == 2) x = -h;
+                        else if (d == 2) x = hg;
+                        else if (d == -2) x = -gam;
+                    }
+                    if (p == pp) x = __dsub_rn(x, Kw);
+                    val[e] = x;
+                }
+                *reinterpret_cast<double2 *>(&W[(size_t)(4 * bmc + pp) * ld + rb + 2 * lane]) = make_double2(val[0], val[1]);
+            }
+        }
+    }
+}
+
+template <bool DMMA_UPD, bool DUMP>
+__global__ void __launch_bounds__(32)
+factor_wc_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_cell, double *__restrict__ dumpA, int dump_cell,
+                 int /* role_mode: factor_wc2_kernel only */)
+{
+    constexpr int n = 64, LD = WC_LD, NPANEL = n / FR_NB;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) unsigned char wc_smem[];
+    WcShared &sh = *reinterpret_cast<WcShared *>(wc_smem);
+    double *W = sh.W;
+    const int lane = threadIdx.x, lq = lane & 3, lg = lane >> 2;
+
+    for (;;) {
+        int cell = dump_cell;
+        if (!DUMP) {
+            if (lane == 0) cell = atomicAdd(next_cell, 1);
+            cell = __shfl_sync(FULL, cell, 0);
+        }
+        if (cell >= P.J) break;
+        assemble_rows2(P, cell, lane, W, LD);
+        __syncwarp();
+        if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
+            for (int e = lane; e < n * n; e += 32) dumpA[e] = W[(e & 63) * LD + (e >> 6)];
+            break;
+        }
+
+        bool used0 = false, used1 = false; // rows 2 lane, 2 lane + 1 have been pivot rows
+        bool singular = false;
+        for (int pnl = 0; pnl < NPANEL; ++pnl) {
+            // ================= phase P: the 64 x 8 panel in registers, two rows per lane =================
+            double t[FR_NB][2];
+#pragma unroll
+            for (int c = 0; c < FR_NB; ++c) {
+                const double2 v = *reinterpret_cast<const double2 *>(&W[(FR_NB * pnl + c) * LD + 2 * lane]);
+                t[c][0] = v.x;
+                t[c][1] = v.y;
+            }
+            int Rl[FR_NB];
+            bool bad = false;
+#pragma unroll
+            for (int b = 0; b < FR_NB; ++b) {
+                const unsigned long long key0 = used0 ? 0ull : (unsigned long long)__double_as_longlong(fabs(t[b][0]));
+                const unsigned long long key1 = used1 ? 0ull : (unsigned long long)__double_as_longlong(fabs(t[b][1]));
+                const bool e1 = key1 > key0; // the lane's own winner: the lower row on a tie
+                const unsigned long long key = e1 ? key1 : key0;
+                const unsigned khi = (unsigned)(key >> 32);
+                const unsigned mhi = __reduce_max_sync(FULL, khi);
+                const unsigned eball = __ballot_sync(FULL, e1);
+                // in the shadow of the reduction: the lane's candidate row scaled by 1 / its candidate
+                double tl[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) tl[c] = e1 ? t[c][1] : t[c][0];
+                const double linv = rcp_nr(tl[b]);
+                double scl[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) scl[c] = (c == b) ? linv : tl[c] * linv;
+                bool cand = khi == mhi;
+                const unsigned ball = __ballot_sync(FULL, cand);
+                int src;
+                if (__popc(ball) == 1) {
+                    src = __ffs(ball) - 1;
+                } else { // ties in the high word: low words, then the lowest lane (= the lowest row)
+                    const unsigned klo = (unsigned)key;
+                    const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
+                    cand = cand && klo == mlo;
+                    const unsigned b2 = __ballot_sync(FULL, cand);
+                    src = b2 ? __ffs(b2) - 1 : 0;
+                }
+                if (mhi == 0u || mhi >= 0x7ff00000u) bad = true; // zero / denormal / inf / NaN pivot (or no unused row)
+                const int esrc = (eball >> src) & 1;
+                if (lane == src) {
+                    double2 *dst = reinterpret_cast<double2 *>(sh.prow[b & 1]);
+#pragma unroll
+                    for (int c = 0; c < FR_NB / 2; ++c) dst[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
+                }
+                __syncwarp(); // (two buffers alternate: no second barrier needed)
+                double sp[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB / 2; ++c) {
+                    const double2 v = reinterpret_cast<const double2 *>(sh.prow[b & 1])[c];
+                    sp[2 * c] = v.x;
+                    sp[2 * c + 1] = v.y;
+                }
+                Rl[b] = 2 * src + esrc;
+                const bool p0 = lane == src && esrc == 0, p1 = lane == src && esrc == 1;
+                const double f0 = t[b][0], f1 = t[b][1];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) { // the pivot row becomes itself / pivot (= scl)
+                    const double u0 = (c == b) ? -f0 * sp[b] : fma(-f0, sp[c], t[c][0]);
+                    const double u1 = (c == b) ? -f1 * sp[b] : fma(-f1, sp[c], t[c][1]);
+                    t[c][0] = p0 ? scl[c] : u0;
+                    t[c][1] = p1 ? scl[c] : u1;
+                }
+                used0 = used0 || p0;
+                used1 = used1 || p1;
+                if (lane == b) { sh.rho[FR_NB * pnl + b] = Rl[b]; sh.rhoinv[Rl[b]] = FR_NB * pnl + b; }
+            }
+            if (bad) { singular = true; break; } // warp-uniform
+            // the eliminated panel (its columns now hold T e_r) back in place
+#pragma unroll
+            for (int c = 0; c < FR_NB; ++c)
+                *reinterpret_cast<double2 *>(&W[(FR_NB * pnl + c) * LD + 2 * lane]) = make_double2(t[c][0], t[c][1]);
+            __syncwarp();
+
+            // ================= phase U: rank-8 update of the other 56 columns =================
+            if (DMMA_UPD) {
+                const int rk0 = sh.rho[FR_NB * pnl + lq], rk1 = sh.rho[FR_NB * pnl + 4 + lq];
+                double af[8][2]; // A fragments: Z[8 I + lg][4 h + lq]
+#pragma unroll
+                for (int I = 0; I < 8; ++I) {
+                    const int row = 8 * I + lg;
+                    af[I][0] = W[(FR_NB * pnl + lq) * LD + row] - (rk0 == row ? 1.0 : 0.0);
+                    af[I][1] = W[(FR_NB * pnl + 4 + lq) * LD + row] - (rk1 == row ? 1.0 : 0.0);
+                }
+                for (int Jb = 0; Jb < 8; ++Jb) {
+                    if (Jb == pnl) continue;
+                    // B fragments: W_old[R[4 h + lq]][8 Jb + lg], read before any lane touches this column block
+                    const double bf0 = W[(8 * Jb + lg) * LD + rk0], bf1 = W[(8 * Jb + lg) * LD + rk1];
+                    __syncwarp();
+                    double *cp = &W[(8 * Jb + 2 * lq) * LD + lg];
+#pragma unroll
+                    for (int I = 0; I < 8; ++I) {
+                        double c0 = cp[8 * I], c1 = cp[LD + 8 * I];
+                        dmma884(c0, c1, af[I][0], bf0);
+                        dmma884(c0, c1, af[I][1], bf1);
+                        cp[8 * I] = c0;
+                        cp[LD + 8 * I] = c1;
+                    }
+                }
+            } else {
+                double z[FR_NB][2];
+#pragma unroll
+                for (int b = 0; b < FR_NB; ++b) {
+                    z[b][0] = t[b][0] - (Rl[b] == 2 * lane ? 1.0 : 0.0);
+                    z[b][1] = t[b][1] - (Rl[b] == 2 * lane + 1 ? 1.0 : 0.0);
+                }
+                for (int c = 0; c < n; ++c) {
+                    if ((c >> 3) == pnl) continue;
+                    double rv[FR_NB];
+#pragma unroll
+                    for (int b = 0; b < FR_NB; ++b) rv[b] = W[c * LD + Rl[b]]; // uniform address
+                    double2 v = *reinterpret_cast<const double2 *>(&W[c * LD + 2 * lane]);
+                    __syncwarp(); // every lane has read the pivot rows of this column
+#pragma unroll
+                    for (int b = 0; b < FR_NB; ++b) { v.x = fma(z[b][0], rv[b], v.x); v.y = fma(z[b][1], rv[b], v.y); }
+                    *reinterpret_cast<double2 *>(&W[c * LD + 2 * lane]) = v;
+                }
+            }
+            __syncwarp();
+        }
+
+        double *out = Minv + (size_t)cell * n * n;
+        if (singular) {
+            if (lane == 0) atomicMin(info, cell + 1);
+            for (int e = lane; e < n * n / 2; e += 32) reinterpret_cast<double2 *>(out)[e] = make_double2(0.0, 0.0);
+            __syncwarp();
+            continue;
+        }
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j], i.e. out[c][r] = W[rho[r]][rhoinv[c]]
+        const int i0 = sh.rho[2 * lane], i1 = sh.rho[2 * lane + 1];
+#pragma unroll 4
+        for (int c = 0; c < n; ++c) {
+            const double *col = &W[sh.rhoinv[c] * LD];
+            reinterpret_cast<double2 *>(out + (size_t)c * n)[lane] = make_double2(col[i0], col[i1]);
+        }
+        __syncwarp(); // every lane is done with W before the next cell's assembly overwrites it
+    }
+}
+
+// ============================================================================================================
+// n = 64, TWO WARPS PER CELL with look-ahead: the production a1 + a2 kernel of the headline configuration.
+// ============================================================================================================
+// Same data layout and arithmetic as factor_wc_kernel. ncu on that kernel (profiles/r02_factor.md): a warp that
+// issues a DMMA cannot issue anything else for ~15 cycles, so the rank-8 update of one warp takes 16 cycles per DMMA
+// whatever else there is to overlap, and phase U was 40 % of a cell's latency. Here warp A runs the pivot chain and
+// warp B the updates: after panel p is eliminated, A updates ONLY column block p + 1 and goes straight on to
+// eliminate it, while B applies update p to the other six blocks -- the classic look-ahead of blocked LU. One CTA
+// barrier per panel (A: Z(p) is in shared memory; B: update p - 1 is complete). The critical path of a cell is its
+// 64 pivot steps plus eight one-block updates; six cells (twelve warps) per SM.
+// Fragment rows: the two 8 x 8 tiles of a 16-row group take the even / the odd rows of the group, so a lane's two
+// tiles are adjacent in a column and accumulators and A fragments move as 16-byte accesses (any permutation of the M
+// dimension of a matrix product is free).
+constexpr int WC2_LD = 72; // 72 = 8 mod 16: the two columns of a quarter-warp's 16-byte accumulator access hit disjoint banks
+
+struct Wc2Shared {
+    double W[64 * WC2_LD];         // [column][row], column-major working matrix
+    double prow[2][FR_NB + 2];     // [step parity]: the pivot row of the current step as it stands, then 1 / pivot
+    int rho[64], rhoinv[64];
+    int cell, sing;
+};
+
+// Rank-8 update of column block Jb (8 columns) from the panel whose pivot rows are rk0 = R[lq], rk1 = R[4 + lq]:
+// W[:, 8 Jb ..] += Z W_old[R, 8 Jb ..], Z = T[:, R] - I[:, R], evaluated TRANSPOSED so that a lane's two accumulators
+// are adjacent rows of one column (one 16-byte access): D[i][j] += sum_k A[i][k] B[k][j] with
+//   A[i][k] = W_old[R[k]][8 Jb + i]   (lane holds A[lg][lq]),   B[k][j] = T[8 I + j][R-column k]   (lane holds B[lq][lg]),
+//   D[i][j] = W[8 I + j][8 Jb + i]    (lane holds rows 8 I + 2 lq, + 1 of column 8 Jb + lg).
+// The "- I[:, R]" costs nothing: row r_b of the result is sum_k T[r_b][k] W_old[R[k]][c] WITHOUT its own old value, so
+// the eight pivot rows of the block are zeroed (by the lanes that have just read them as A fragments) before the
+// accumulators are loaded, and the B fragments are the eliminated panel as it stands in W.
+template <int NBLK>
+__device__ __forceinline__ void wc2_update_blocks(double *W, const int (&Jb)[NBLK], const double (&zf)[8][2], int rk0, int rk1,
+                                                  int lq, int lg)
+{
+    constexpr int LD = WC2_LD;
+    // A fragments of all the blocks first (then they are zeroed, see above): one pair of warp barriers for the lot, and
+    // nothing but loads, DMMAs and stores of independent tiles afterwards
+    double a0[NBLK], a1[NBLK];
+#pragma unroll
+    for (int i = 0; i < NBLK; ++i) {
+        a0[i] = W[(8 * Jb[i] + lg) * LD + rk0];
+        a1[i] = W[(8 * Jb[i] + lg) * LD + rk1];
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < NBLK; ++i) {
+        W[(8 * Jb[i] + lg) * LD + rk0] = 0.0;
+        W[(8 * Jb[i] + lg) * LD + rk1] = 0.0;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < NBLK; ++i) {
+        double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb[i] + lg) * LD + 2 * lq]);
+#pragma unroll
+        for (int I = 0; I < 8; ++I) {
+            double2 v = cp[4 * I];
+            dmma884(v.x, v.y, a0[i], zf[I][0]);
+            dmma884(v.x, v.y, a1[i], zf[I][1]);
+            cp[4 * I] = v;
+        }
+    }
+}
+
+// One pivot step (column b of the panel) of warp A: rows {2 lane, 2 lane + 1} as two row vectors in registers.
+struct WcPanel {
+    double t0[FR_NB], t1[FR_NB]; // row 2 lane, row 2 lane + 1
+    unsigned m0, m1;             // 0x7fffffff while the row is unused, 0 once it has been a pivot row
+};
+
+template <int b>
+__device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, int *rho, int *rhoinv, int col0, int lane,
+                                               unsigned &bad)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    // |entry| of the unused rows as integer keys (non-negative doubles order like their bit patterns); the low words
+    // need no mask: a used row can only win with a zero high word, and that is flagged as singular anyway
+    const unsigned h0 = (unsigned)__double2hiint(R.t0[b]) & R.m0, h1 = (unsigned)__double2hiint(R.t1[b]) & R.m1;
+    const unsigned l0 = (unsigned)__double2loint(R.t0[b]), l1 = (unsigned)__double2loint(R.t1[b]);
+    const bool e1 = h1 > h0 || (h1 == h0 && l1 > l0); // the lane's own winner: the lower row on a tie
+    const unsigned khi = e1 ? h1 : h0;
+    const unsigned mhi = __reduce_max_sync(FULL, khi);
+    const unsigned eball = __ballot_sync(FULL, e1);
+    const double linv = rcp_nr(e1 ? R.t1[b] : R.t0[b]); // in the shadow of the reduction: 1 / (the lane's candidate)
+    unsigned ball = __ballot_sync(FULL, khi == mhi);
+    if (__popc(ball) != 1) { // ties in the high word: low words, then the lowest lane (= the lowest row)
+        const unsigned klo = e1 ? l1 : l0;
+        const bool cand = khi == mhi;
+        const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
+        ball = __ballot_sync(FULL, cand && klo == mlo);
+    }
+    const int src = __ffs(ball) - 1;
+    bad |= (mhi - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot, or no unused row left
+    const int esrc = (eball >> (src & 31)) & 1;
+    const bool p0 = lane == src && esrc == 0, p1 = lane == src && esrc != 0;
+    double *pr = prow_base + (b & 1) * (FR_NB + 2);
+    // the winner publishes its row as it stands, and 1 / pivot
+    if (p0) {
+#pragma unroll
+        for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(pr)[c] = make_double2(R.t0[2 * c], R.t0[2 * c + 1]);
+        pr[FR_NB] = linv;
+    }
+    if (p1) {
+#pragma unroll
+        for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(pr)[c] = make_double2(R.t1[2 * c], R.t1[2 * c + 1]);
+        pr[FR_NB] = linv;
+    }
+    __syncwarp(); // (two buffers alternate: no second barrier needed)
+    const double ls = pr[FR_NB];
+    double sp[FR_NB]; // pivot row / pivot; column b holds 1 / pivot
+#pragma unroll
+    for (int c = 0; c < FR_NB / 2; ++c) {
+        const double2 v = reinterpret_cast<const double2 *>(pr)[c];
+        sp[2 * c] = (2 * c == b) ? ls : v.x * ls;
+        sp[2 * c + 1] = (2 * c + 1 == b) ? ls : v.y * ls;
+    }
+    const double f0 = R.t0[b], f1 = R.t1[b];
+#pragma unroll
+    for (int c = 0; c < FR_NB; ++c) {
+        R.t0[c] = (c == b) ? -f0 * ls : fma(-f0, sp[c], R.t0[c]);
+        R.t1[c] = (c == b) ? -f1 * ls : fma(-f1, sp[c], R.t1[c]);
+    }
+    // the pivot row becomes itself / pivot (predicated moves: a divergent branch would add its resolve and
+    // reconvergence latency to the chain)
+    if (p0) {
+#pragma unroll
+        for (int c = 0; c < FR_NB; ++c) R.t0[c] = sp[c];
+        R.m0 = 0u;
+    }
+    if (p1) {
+#pragma unroll
+        for (int c = 0; c < FR_NB; ++c) R.t1[c] = sp[c];
+        R.m1 = 0u;
+    }
+    if (lane == b) {
+        const int r = 2 * src + esrc;
+        rho[col0 + b] = r;
+        rhoinv[r & 63] = col0 + b;
+    }
+}
+
+template <bool DUMP>
+__global__ void __launch_bounds__(64)
+factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_cell, double *__restrict__ dumpA, int dump_cell,
+                  int role_mode)
+{
+    constexpr int n = 64, LD = WC2_LD, NPANEL = n / FR_NB;
+    extern __shared__ __align__(16) unsigned char wc_smem[];
+    Wc2Shared &sh = *reinterpret_cast<Wc2Shared *>(wc_smem);
+    double *W = sh.W;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
+    // Role: warp A runs the pivot chain, warp B the updates. The two warps of a CTA sit on neighbouring SM
+    // sub-partitions (warp slots 2 k, 2 k + 1: measured); alternating the roles with bit 2 of the slot puts the six A
+    // warps of an SM on all four schedulers instead of two.
+    unsigned slot;
+    asm("mov.u32 %0, %%warpid;" : "=r"(slot));
+    const bool roleA = role_mode ? w == 0 : ((slot ^ (slot >> 2)) & 1u) == 0u;
+
+    for (;;) {
+        if (threadIdx.x == 0) { sh.cell = DUMP ? dump_cell : atomicAdd(next_cell, 1); sh.sing = 0; }
+        __syncthreads();
+        const int cell = sh.cell;
+        if (cell >= P.J) break;
+        assemble_rows2(P, cell, lane, W, LD, w, 2);
+        __syncthreads();
+        if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
+            for (int e = threadIdx.x; e < n * n; e += 64) dumpA[e] = W[(e & 63) * LD + (e >> 6)];
+            break;
+        }
+
+        WcPanel R;
+        R.m0 = R.m1 = 0x7fffffffu;
+        bool singular = false;
+        for (int pnl = 0; pnl < NPANEL; ++pnl) {
+            if (roleA) {
+                // ================= phase P (warp A): the 64 x 8 panel in registers, two rows per lane =================
+                double *Wp = &W[(FR_NB * pnl) * LD + 2 * lane];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) {
+                    const double2 v = *reinterpret_cast<const double2 *>(Wp + c * LD);
+                    R.t0[c] = v.x;
+                    R.t1[c] = v.y;
+                }
+                unsigned bad = 0u;
+                wc2_pivot_step<0>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<1>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<2>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<3>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<4>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<5>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<6>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                wc2_pivot_step<7>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                if (bad && lane == 0) sh.sing = 1;
+                // the eliminated panel (its columns now hold T e_r) back in place
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) *reinterpret_cast<double2 *>(Wp + c * LD) = make_double2(R.t0[c], R.t1[c]);
+            }
+            __syncthreads(); // barrier p: Z(p), R(p) visible to B; B has completed update p - 1
+            if (sh.sing) { singular = true; break; } // CTA-uniform
+
+            // ================= phase U: rank-8 update of the other 56 columns =================
+            const int rk0 = sh.rho[FR_NB * pnl + lq], rk1 = sh.rho[FR_NB * pnl + 4 + lq];
+            double zf[8][2]; // B fragments: T[8 I + lg][panel column 4 h + lq]
+#pragma unroll
+            for (int I = 0; I < 8; ++I) {
+                zf[I][0] = W[(FR_NB * pnl + lq) * LD + 8 * I + lg];
+                zf[I][1] = W[(FR_NB * pnl + 4 + lq) * LD + 8 * I + lg];
+            }
+            if (pnl + 1 < NPANEL) { // A: the next panel's block only (then straight on to eliminate it); B: the rest
+                if (roleA) {
+                    const int jb[1] = {pnl + 1};
+                    wc2_update_blocks<1>(W, jb, zf, rk0, rk1, lq, lg);
+                    __syncwarp();
+                } else {
+                    int jb[6];
+#pragma unroll
+                    for (int i = 0; i < 6; ++i) jb[i] = i < pnl ? i : i + 2;
+                    wc2_update_blocks<6>(W, jb, zf, rk0, rk1, lq, lg);
+                }
+            } else { // last panel: blocks 0..6 shared out
+                if (w == 0) {
+                    const int jb[4] = {0, 2, 4, 6};
+                    wc2_update_blocks<4>(W, jb, zf, rk0, rk1, lq, lg);
+                } else {
+                    const int jb[3] = {1, 3, 5};
+                    wc2_update_blocks<3>(W, jb, zf, rk0, rk1, lq, lg);
+                }
+            }
+        }
+        __syncthreads(); // update 7 complete
+
+        double *out = Minv + (size_t)cell * n * n;
+        if (singular) {
+            if (threadIdx.x == 0) atomicMin(info, cell + 1);
+            for (int e = threadIdx.x; e < n * n / 2; e += 64) reinterpret_cast<double2 *>(out)[e] = make_double2(0.0, 0.0);
+            __syncthreads();
+            continue;
+        }
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j], i.e. out[c][r] = W[rho[r]][rhoinv[c]]
+        const int i0 = sh.rho[2 * lane], i1 = sh.rho[2 * lane + 1];
+#pragma unroll 4
+        for (int c = w; c < n; c += 2) {
+            const double *col = &W[sh.rhoinv[c] * LD];
+            reinterpret_cast<double2 *>(out + (size_t)c * n)[lane] = make_double2(col[i0], col[i1]);
+        }
+        __syncthreads(); // everybody is done with W and sh.cell before the next cell
+    }
+}
+
 __global__ void assemble_one_kernel(ProblemView P, int cell, double *__restrict__ A)
 {
     const int n = P.n;
@@ -697,12 +1203,45 @@ template <int NQ> static int launch_factor_reg(oci_ctx *ctx, const ProblemView &
     return 1;
 }
 
+// n = 64, one warp per cell (factor_wc_kernel). dumpA != nullptr: only assemble `dump_cell` and write the tile there.
+static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
+{
+    const bool two = ctx->opt_factor_kernel == 1; // 1: two warps per cell with look-ahead; 4: one warp per cell
+    const size_t smem = two ? sizeof(Wc2Shared) : sizeof(WcShared);
+    const int threads = two ? 64 : 32;
+    const bool dmma = ctx->opt_factor_update != 0;
+    const void *fn;
+    if (two) fn = dumpA ? (const void *)factor_wc2_kernel<true> : (const void *)factor_wc2_kernel<false>;
+    else fn = dumpA ? (const void *)factor_wc_kernel<true, true>
+                    : (dmma ? (const void *)factor_wc_kernel<true, false> : (const void *)factor_wc_kernel<false, false>);
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    int grid = 1;
+    if (!dumpA) {
+        int per_sm = 0;
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem));
+        if (ctx->opt_factor_update >= 10 && ctx->opt_factor_update - 10 < per_sm) per_sm = ctx->opt_factor_update - 10; // probe
+        grid = (per_sm < 1 ? 1 : per_sm) * ctx->num_sms;
+        if (grid > ctx->J) grid = ctx->J;
+        OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info + 1, 0, sizeof(int), ctx->stream)); // the cell counter
+    }
+    int *counter = ctx->info + 1;
+    double *Minv = ctx->Minv;
+    int *info = ctx->info;
+    ProblemView Pv = P;
+    int role_mode = ctx->opt_factor_update == 2 ? 1 : 0; // (tuning probe) 2: warp 0 is always the pivot warp
+    void *args[] = {&Pv, &Minv, &info, &counter, &dumpA, &dump_cell, &role_mode};
+    OCI_CUDA_TRY(ctx, cudaLaunchKernel(fn, dim3(grid), dim3(threads), args, smem, ctx->stream));
+    return 1;
+}
+
 int launch_factor(oci_ctx *ctx)
 {
     const int n = ctx->n;
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream)); // 0x7f7f7f7f = "none"
-    if (ctx->opt_factor_kernel == 1 && n == 64) {
+    if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && n == 64) return launch_factor_wc(ctx, P, nullptr, 0);
+    if (ctx->opt_factor_kernel == 3 && n == 64) { // the register-resident two-warp kernel of round 1 (kept for the A/B)
         int per_sm = 0;
         const size_t smem = sizeof(W2Shared);
         OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_w2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -742,6 +1281,16 @@ int launch_factor(oci_ctx *ctx)
     }
     OCI_CUDA_TRY(ctx, cudaGetLastError());
     return 1;
+}
+
+// The tile the production factor kernel of the current options assembles on chip for `cell`, dumped before the
+// elimination (row-major); 0 = that kernel has no such path (it assembles through a_entry(), see launch_assemble_one).
+int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor)
+{
+    ProblemView P = make_view(ctx);
+    if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && ctx->n == 64)
+        return launch_factor_wc(ctx, P, A_dev_rowmajor, cell);
+    return 0;
 }
 
 int launch_assemble_one(oci_ctx *ctx, int cell, double *A_dev_rowmajor)

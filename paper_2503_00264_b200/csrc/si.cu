@@ -415,8 +415,10 @@ si_finish_kernel(StopCheck stop, int J, int N, int G, const double *__restrict__
             }
         }
         __syncthreads();
-        const int lp = tid >> 2, p = tid & 3;
-        if (lp < pairs_per_block && pair0 + lp < n_pairs) {
+        // N = 2 gives 128 pairs per block = 512 (pair, p) entries: stride over them (one pass for N >= 4)
+        for (int t = tid; t < pairs_per_block * 4; t += FIN_THREADS) {
+            const int lp = t >> 2, p = t & 3;
+            if (pair0 + lp >= n_pairs) break;
             double s = 0.0;
             for (int mm = 0; mm < N; ++mm) s += ws[lp * N + mm][p];
             const size_t o = (pair0 + lp) * 4 + p;
