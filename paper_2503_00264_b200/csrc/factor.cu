@@ -908,7 +908,13 @@ factor_wc_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_
 // Fragment rows: the two 8 x 8 tiles of a 16-row group take the even / the odd rows of the group, so a lane's two
 // tiles are adjacent in a column and accumulators and A fragments move as 16-byte accesses (any permutation of the M
 // dimension of a matrix product is free).
-constexpr int WC2_LD = 72; // 72 = 8 mod 16: the two columns of a quarter-warp's 16-byte accumulator access hit disjoint banks
+// Leading dimension 68 (= 4 mod 16: a column starts 8 banks after its neighbour) and the columns of a block taken in the
+// order 0 2 1 3 4 6 5 7 by the eight lane groups (any permutation of the M dimension of a product is free): the two
+// columns of a quarter-warp's 16-byte accumulator access are then 16 banks apart, and the four panel columns of a
+// half-warp's B-fragment load 8 banks apart -- both conflict-free (LD = 72 made the second a two-way conflict, and
+// shared-memory wavefronts are what this kernel saturates: ncu l1tex__data_pipe_lsu_wavefronts_mem_shared 73 %).
+constexpr int WC2_LD = 68;
+__device__ __forceinline__ int wc2_colmap(int lg) { return (lg & 4) | ((lg & 1) << 1) | ((lg >> 1) & 1); }
 
 struct Wc2Shared {
     double W[64 * WC2_LD];         // [column][row], column-major working matrix
@@ -920,8 +926,8 @@ struct Wc2Shared {
 // Rank-8 update of column block Jb (8 columns) from the panel whose pivot rows are rk0 = R[lq], rk1 = R[4 + lq]:
 // W[:, 8 Jb ..] += Z W_old[R, 8 Jb ..], Z = T[:, R] - I[:, R], evaluated TRANSPOSED so that a lane's two accumulators
 // are adjacent rows of one column (one 16-byte access): D[i][j] += sum_k A[i][k] B[k][j] with
-//   A[i][k] = W_old[R[k]][8 Jb + i]   (lane holds A[lg][lq]),   B[k][j] = T[8 I + j][R-column k]   (lane holds B[lq][lg]),
-//   D[i][j] = W[8 I + j][8 Jb + i]    (lane holds rows 8 I + 2 lq, + 1 of column 8 Jb + lg).
+//   A[i][k] = W_old[R[k]][8 Jb + c(i)] (lane holds A[lg][lq]),  B[k][j] = T[8 I + j][R-column k]   (lane holds B[lq][lg]),
+//   D[i][j] = W[8 I + j][8 Jb + c(i)]  (lane holds rows 8 I + 2 lq, + 1 of column 8 Jb + c(lg)), c = wc2_colmap.
 // The "- I[:, R]" costs nothing: row r_b of the result is sum_k T[r_b][k] W_old[R[k]][c] WITHOUT its own old value, so
 // the eight pivot rows of the block are zeroed (by the lanes that have just read them as A fragments) before the
 // accumulators are loaded, and the B fragments are the eliminated panel as it stands in W.
@@ -932,22 +938,23 @@ __device__ __forceinline__ void wc2_update_blocks(double *W, const int (&Jb)[NBL
     constexpr int LD = WC2_LD;
     // A fragments of all the blocks first (then they are zeroed, see above): one pair of warp barriers for the lot, and
     // nothing but loads, DMMAs and stores of independent tiles afterwards
+    const int cl = wc2_colmap(lg); // this lane group's column of a block
     double a0[NBLK], a1[NBLK];
 #pragma unroll
     for (int i = 0; i < NBLK; ++i) {
-        a0[i] = W[(8 * Jb[i] + lg) * LD + rk0];
-        a1[i] = W[(8 * Jb[i] + lg) * LD + rk1];
+        a0[i] = W[(8 * Jb[i] + cl) * LD + rk0];
+        a1[i] = W[(8 * Jb[i] + cl) * LD + rk1];
     }
     __syncwarp();
 #pragma unroll
     for (int i = 0; i < NBLK; ++i) {
-        W[(8 * Jb[i] + lg) * LD + rk0] = 0.0;
-        W[(8 * Jb[i] + lg) * LD + rk1] = 0.0;
+        W[(8 * Jb[i] + cl) * LD + rk0] = 0.0;
+        W[(8 * Jb[i] + cl) * LD + rk1] = 0.0;
     }
     __syncwarp();
 #pragma unroll
     for (int i = 0; i < NBLK; ++i) {
-        double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb[i] + lg) * LD + 2 * lq]);
+        double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb[i] + cl) * LD + 2 * lq]);
 #pragma unroll
         for (int I = 0; I < 8; ++I) {
             double2 v = cp[4 * I];
@@ -959,14 +966,28 @@ __device__ __forceinline__ void wc2_update_blocks(double *W, const int (&Jb)[NBL
 }
 
 // One pivot step (column b of the panel) of warp A: rows {2 lane, 2 lane + 1} as two row vectors in registers.
+// 8-byte shared-memory load the compiler may not fuse with its neighbour into a 16-byte one (a 16-byte broadcast
+// load costs 2.5 wavefronts, two 8-byte ones 2)
+__device__ __forceinline__ double lds_f64(const double *p)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(smem_u32(p)));
+    return v;
+}
+
 struct WcPanel {
     double t0[FR_NB], t1[FR_NB]; // row 2 lane, row 2 lane + 1
     unsigned m0, m1;             // 0x7fffffff while the row is unused, 0 once it has been a pivot row
 };
 
-template <int b>
+// FAST = true is the optimistic form the kernel runs first: no branch (the eight steps of a panel are ONE basic block, so
+// the scheduler overlaps the tail of a step with the reduction of the next), a tie of the high key words is only
+// RECORDED, and the one column the next pivot decision depends on travels by shuffle instead of through shared memory.
+// If a panel recorded a tie it is reloaded and eliminated again with FAST = false, which resolves ties exactly (low key
+// words, then the lowest row: the first maximal |entry|, as LAPACK's idamax). Same arithmetic in both forms.
+template <int b, bool FAST>
 __device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, int *rho, int *rhoinv, int col0, int lane,
-                                               unsigned &bad)
+                                               unsigned &bad, unsigned &tie)
 {
     constexpr unsigned FULL = 0xffffffffu;
     // |entry| of the unused rows as integer keys (non-negative doubles order like their bit patterns); the low words
@@ -979,40 +1000,54 @@ __device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, in
     const unsigned eball = __ballot_sync(FULL, e1);
     const double linv = rcp_nr(e1 ? R.t1[b] : R.t0[b]); // in the shadow of the reduction: 1 / (the lane's candidate)
     unsigned ball = __ballot_sync(FULL, khi == mhi);
-    if (__popc(ball) != 1) { // ties in the high word: low words, then the lowest lane (= the lowest row)
+    if (FAST) {
+        tie |= ball & (ball - 1u); // more than one lane holds the maximal high word
+    } else if (__popc(ball) != 1) { // ties in the high word: low words, then the lowest lane (= the lowest row)
         const unsigned klo = e1 ? l1 : l0;
         const bool cand = khi == mhi;
         const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
         ball = __ballot_sync(FULL, cand && klo == mlo);
     }
-    const int src = __ffs(ball) - 1;
+    const int src = (__ffs(ball) - 1) & 31;
     bad |= (mhi - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot, or no unused row left
-    const int esrc = (eball >> (src & 31)) & 1;
+    const int esrc = (eball >> src) & 1;
     const bool p0 = lane == src && esrc == 0, p1 = lane == src && esrc != 0;
+    const double f0 = R.t0[b], f1 = R.t1[b];
+    double ls;
+    if (FAST) { // 1 / pivot and, below, column b + 1 of the pivot row by shuffle: nothing else is on the critical path
+        ls = __shfl_sync(FULL, linv, src);
+        if (b + 1 < FR_NB) {
+            const double xn = __shfl_sync(FULL, esrc ? R.t1[b + 1] : R.t0[b + 1], src) * ls;
+            const double u0 = fma(-f0, xn, R.t0[b + 1]), u1 = fma(-f1, xn, R.t1[b + 1]);
+            R.t0[b + 1] = p0 ? xn : u0;
+            R.t1[b + 1] = p1 ? xn : u1;
+        }
+    }
     double *pr = prow_base + (b & 1) * (FR_NB + 2);
-    // the winner publishes its row as it stands, and 1 / pivot
+    // the winner publishes its row as it stands (and 1 / pivot for the exact form)
     if (p0) {
 #pragma unroll
         for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(pr)[c] = make_double2(R.t0[2 * c], R.t0[2 * c + 1]);
-        pr[FR_NB] = linv;
+        if (!FAST) pr[FR_NB] = linv;
     }
     if (p1) {
 #pragma unroll
         for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(pr)[c] = make_double2(R.t1[2 * c], R.t1[2 * c + 1]);
-        pr[FR_NB] = linv;
+        if (!FAST) pr[FR_NB] = linv;
     }
     __syncwarp(); // (two buffers alternate: no second barrier needed)
-    const double ls = pr[FR_NB];
-    double sp[FR_NB]; // pivot row / pivot; column b holds 1 / pivot
-#pragma unroll
-    for (int c = 0; c < FR_NB / 2; ++c) {
-        const double2 v = reinterpret_cast<const double2 *>(pr)[c];
-        sp[2 * c] = (2 * c == b) ? ls : v.x * ls;
-        sp[2 * c + 1] = (2 * c + 1 == b) ? ls : v.y * ls;
-    }
-    const double f0 = R.t0[b], f1 = R.t1[b];
+    if (!FAST) ls = pr[FR_NB];
+    double sp[FR_NB]; // pivot row / pivot; column b holds 1 / pivot. 8-byte broadcast loads (one wavefront each) of the
+                      // columns that are still needed: shared-memory wavefronts are the resource this kernel saturates
 #pragma unroll
     for (int c = 0; c < FR_NB; ++c) {
+        if (c == b) sp[c] = ls;
+        else if (FAST && c == b + 1) sp[c] = 0.0; // (unused)
+        else sp[c] = lds_f64(pr + c) * ls;
+    }
+#pragma unroll
+    for (int c = 0; c < FR_NB; ++c) {
+        if (FAST && c == b + 1) continue; // done above (the published row still holds its old value of that column)
         R.t0[c] = (c == b) ? -f0 * ls : fma(-f0, sp[c], R.t0[c]);
         R.t1[c] = (c == b) ? -f1 * ls : fma(-f1, sp[c], R.t1[c]);
     }
@@ -1020,25 +1055,41 @@ __device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, in
     // reconvergence latency to the chain)
     if (p0) {
 #pragma unroll
-        for (int c = 0; c < FR_NB; ++c) R.t0[c] = sp[c];
+        for (int c = 0; c < FR_NB; ++c)
+            if (!(FAST && c == b + 1)) R.t0[c] = sp[c];
         R.m0 = 0u;
     }
     if (p1) {
 #pragma unroll
-        for (int c = 0; c < FR_NB; ++c) R.t1[c] = sp[c];
+        for (int c = 0; c < FR_NB; ++c)
+            if (!(FAST && c == b + 1)) R.t1[c] = sp[c];
         R.m1 = 0u;
     }
     if (lane == b) {
         const int r = 2 * src + esrc;
         rho[col0 + b] = r;
-        rhoinv[r & 63] = col0 + b;
+        rhoinv[r] = col0 + b;
     }
+}
+
+template <bool FAST>
+__device__ __forceinline__ void wc2_panel(WcPanel &R, double *prow, int *rho, int *rhoinv, int col0, int lane, unsigned &bad,
+                                          unsigned &tie)
+{
+    wc2_pivot_step<0, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<1, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<2, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<3, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<4, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<5, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<6, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    wc2_pivot_step<7, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
 }
 
 template <bool DUMP>
 __global__ void __launch_bounds__(64)
 factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_cell, double *__restrict__ dumpA, int dump_cell,
-                  int role_mode)
+                  int /* unused */)
 {
     constexpr int n = 64, LD = WC2_LD, NPANEL = n / FR_NB;
     extern __shared__ __align__(16) unsigned char wc_smem[];
@@ -1050,7 +1101,7 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
     // warps of an SM on all four schedulers instead of two.
     unsigned slot;
     asm("mov.u32 %0, %%warpid;" : "=r"(slot));
-    const bool roleA = role_mode ? w == 0 : ((slot ^ (slot >> 2)) & 1u) == 0u;
+    const bool roleA = ((slot ^ (slot >> 2)) & 1u) == 0u;
 
     for (;;) {
         if (threadIdx.x == 0) { sh.cell = DUMP ? dump_cell : atomicAdd(next_cell, 1); sh.sing = 0; }
@@ -1077,15 +1128,22 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
                     R.t0[c] = v.x;
                     R.t1[c] = v.y;
                 }
-                unsigned bad = 0u;
-                wc2_pivot_step<0>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<1>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<2>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<3>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<4>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<5>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<6>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
-                wc2_pivot_step<7>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad);
+                unsigned bad = 0u, tie = 0u;
+                const unsigned m0_in = R.m0, m1_in = R.m1;
+                wc2_panel<true>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad, tie);
+                if (tie) { // warp-uniform and rare: the panel again, from shared memory, with exact tie resolution
+#pragma unroll
+                    for (int c = 0; c < FR_NB; ++c) {
+                        const double2 v = *reinterpret_cast<const double2 *>(Wp + c * LD);
+                        R.t0[c] = v.x;
+                        R.t1[c] = v.y;
+                    }
+                    R.m0 = m0_in;
+                    R.m1 = m1_in;
+                    bad = 0u;
+                    __syncwarp();
+                    wc2_panel<false>(R, &sh.prow[0][0], sh.rho, sh.rhoinv, FR_NB * pnl, lane, bad, tie);
+                }
                 if (bad && lane == 0) sh.sing = 1;
                 // the eliminated panel (its columns now hold T e_r) back in place
 #pragma unroll
@@ -1132,12 +1190,16 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
             __syncthreads();
             continue;
         }
-        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j], i.e. out[c][r] = W[rho[r]][rhoinv[c]]
-        const int i0 = sh.rho[2 * lane], i1 = sh.rho[2 * lane + 1];
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]. Column j of W goes to column rho[j] with its
+        // rows scattered by rhoinv: conflict-free 16-byte shared-memory reads, and the 64 eight-byte stores of a column
+        // fill one 512-byte line between them (the L2 merges them: DRAM traffic stays at the 2.09 GB of the result)
+        const int r0 = sh.rhoinv[2 * lane], r1 = sh.rhoinv[2 * lane + 1];
 #pragma unroll 4
-        for (int c = w; c < n; c += 2) {
-            const double *col = &W[sh.rhoinv[c] * LD];
-            reinterpret_cast<double2 *>(out + (size_t)c * n)[lane] = make_double2(col[i0], col[i1]);
+        for (int j = w; j < n; j += 2) {
+            const double2 v = *reinterpret_cast<const double2 *>(&W[j * LD + 2 * lane]);
+            double *col = out + (size_t)sh.rho[j] * n;
+            col[r0] = v.x;
+            col[r1] = v.y;
         }
         __syncthreads(); // everybody is done with W and sh.cell before the next cell
     }
@@ -1220,7 +1282,6 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
     if (!dumpA) {
         int per_sm = 0;
         OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem));
-        if (ctx->opt_factor_update >= 10 && ctx->opt_factor_update - 10 < per_sm) per_sm = ctx->opt_factor_update - 10; // probe
         grid = (per_sm < 1 ? 1 : per_sm) * ctx->num_sms;
         if (grid > ctx->J) grid = ctx->J;
         OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info + 1, 0, sizeof(int), ctx->stream)); // the cell counter
@@ -1229,7 +1290,7 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
     double *Minv = ctx->Minv;
     int *info = ctx->info;
     ProblemView Pv = P;
-    int role_mode = ctx->opt_factor_update == 2 ? 1 : 0; // (tuning probe) 2: warp 0 is always the pivot warp
+    int role_mode = 0;
     void *args[] = {&Pv, &Minv, &info, &counter, &dumpA, &dump_cell, &role_mode};
     OCI_CUDA_TRY(ctx, cudaLaunchKernel(fn, dim3(grid), dim3(threads), args, smem, ctx->stream));
     return 1;
