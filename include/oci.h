@@ -76,17 +76,25 @@ typedef struct {
 size_t oci_workspace_bytes(const oci_problem *p);
 
 /* Validates the problem, carves the workspace, uploads the problem arrays. State starts as psi = 0, q = 0.
- * cuda_stream is a cudaStream_t (NULL = legacy default stream). [sync] */
+ * cuda_stream is a cudaStream_t (NULL = legacy default stream) of the device the workspace lives on. The context is
+ * bound to that device: every later call switches to it for its own duration and restores the caller's current
+ * device, so contexts on several GPUs can be driven from one thread. [sync] */
 int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes, void *cuda_stream,
                oci_ctx **out);
 void oci_destroy(oci_ctx *ctx);
 const char *oci_strerror(int code);
 int oci_last_cuda_error(const oci_ctx *ctx);
+/* cudaError_t behind the most recent oci_create of the calling thread that returned OCI_E_CUDA (0 otherwise): a failed
+ * create returns no context to ask. */
+int oci_last_create_error(void);
 
 /* Tuning knobs (all optional). Known keys: "iterate_kernel" (0 = plain one-CTA-per-cell, 1 = pipelined
  * bulk-copy streaming kernel [default]), "iterate_stages", "iterate_ctas_per_sm", "factor_kernel"
- * (0 = shared-memory elimination, 1 = register-tiled kernels [default]: two warps per cell for n = 64, clusters of
- * n/64 CTAs for n = 128, 192, 256; 2 = the cluster-capable kernel also for n = 64), "solve_mode" (0 = dense
+ * (0 = generic shared-memory elimination, one CTA per cell; 1 = production kernels [default]: for n = 64 the working
+ * matrix in shared memory, one pivot warp + one update warp per cell with look-ahead and rank-8 updates on the FP64
+ * tensor path (DMMA); for n = 128, 192, 256 register-tiled, clusters of n/64 CTAs; 2 = the register-tiled kernel also
+ * for n = 64; 4 = n = 64 with ONE warp per cell, "factor_update" 1 = DMMA [default] or 0 = DFMA rank-8 updates -- the A/B
+ * pair behind DESIGN.md's DMMA decision), "solve_mode" (0 = dense
  * [default]: a2 eliminates the dense A_j with partial pivoting and a5 streams A_j^{-1}, the paper's method;
  * 1 = structured: A_j = D - U V^T with D the 4x4 blocks of Eq. 8b and rank 4G (Eq. 10 / 40b), a2 inverts the
  * blocks and the 4G x 4G capacitance matrix with partial pivoting, a5 applies them -- the same iteration to

@@ -15,7 +15,7 @@ from pathlib import Path
 
 from . import build as _build
 
-__all__ = ["OCISolver", "OCIError", "load_library", "declared_symbols", "BC_VACUUM", "BC_REFLECTIVE",
+__all__ = ["OCISolver", "OCIError", "load_library", "declared_symbols", "create_error", "BC_VACUUM", "BC_REFLECTIVE",
            "BC_PRESCRIBED", "STOP_DPHI_INF", "STOP_PAPER"]
 
 BC_VACUUM, BC_REFLECTIVE, BC_PRESCRIBED = 0, 1, 2
@@ -38,6 +38,7 @@ _SIGNATURES = {
     "oci_destroy": (None, [_dptr]),
     "oci_strerror": (C.c_char_p, [C.c_int]),
     "oci_last_cuda_error": (C.c_int, [_dptr]),
+    "oci_last_create_error": (C.c_int, []),
     "oci_set_option": (C.c_int, [_dptr, C.c_char_p, _i64]),
     "oci_set_dt": (C.c_int, [_dptr, _f64]),
     "oci_set_source": (C.c_int, [_dptr, _dptr]),
@@ -83,6 +84,11 @@ def load_library(rebuild: bool = False):
             fn.restype, fn.argtypes = res, args
         _lib = lib
     return _lib
+
+
+def create_error() -> int:
+    """oci_last_create_error: the cudaError_t behind this thread's most recent failed oci_create (0 if none)."""
+    return int(load_library().oci_last_create_error())
 
 
 class OCIError(RuntimeError):
@@ -135,7 +141,7 @@ class OCISolver:
     # -- plumbing ------------------------------------------------------------------------------------------
     def _check(self, fn: str, code: int, allow_positive: bool = False) -> int:
         if code < 0 or (code > 0 and not allow_positive):
-            cuda = self.lib.oci_last_cuda_error(self._ctx) if self._ctx else 0
+            cuda = self.lib.oci_last_cuda_error(self._ctx) if self._ctx else self.lib.oci_last_create_error()
             raise OCIError(fn, code, cuda)
         return code
 

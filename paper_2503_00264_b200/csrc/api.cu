@@ -2,6 +2,7 @@
 // Alg. 2 (OCI) and Alg. 1 (SI). Host logic only; every numerical step is a
 // kernel in factor.cu / iterate.cu / si.cu.
 #include "common.cuh"
+#include <nvtx3/nvToolsExt.h> // header-only; ranges show up under nsys / ncu --nvtx, and cost nothing otherwise
 #include <math.h>
 #include <new>
 #include <stdlib.h>
@@ -11,6 +12,13 @@
 size_t factor_scratch_bytes(int n, int num_sms, int max_smem_optin);
 
 namespace {
+
+struct NvtxRange { // RAII range on the calling thread (tracing)
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+
+thread_local int g_create_cuda_error = 0; // cudaError_t of the most recent failed oci_create of this thread
 
 constexpr size_t ALIGN = 256;
 inline size_t up(size_t b) { return (b + ALIGN - 1) & ~(ALIGN - 1); }
@@ -26,12 +34,11 @@ struct Carver {
     }
 };
 
-void device_limits(int *num_sms, int *max_smem)
+void device_limits(int *num_sms, int *max_smem, int dev = -1)
 {
     *num_sms = 148;        // B200
     *max_smem = 232448;    // 227 KB opt-in shared memory per CTA on sm_100
-    int dev = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess) {
+    if (dev >= 0 || cudaGetDevice(&dev) == cudaSuccess) {
         int v = 0;
         if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) *num_sms = v;
         if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess && v > 0) *max_smem = v;
@@ -170,6 +177,7 @@ bool rule_holds(int rule, double tol, const double *h_inf, const double *h_l2, i
 int iterate_impl(oci_ctx *ctx, int scheme, int n_iters)
 {
     if (!ctx) return -1;
+    NvtxRange range(scheme == 0 ? "oci_iterate" : "si_iterate");
     if (n_iters < 0) return -2;
     long long launches = 0;
     int r;
@@ -202,6 +210,7 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
     if (max_iters < 1 || max_iters > OCI_RESID_CAP) return -3;
     if (check_every < 1) return -4;
     if (rule != OCI_STOP_DPHI_INF && rule != OCI_STOP_PAPER) return -5;
+    NvtxRange range(scheme == 0 ? "oci_step" : "si_step");
     long long launches = 0;
     int r;
     if (ctx->opt_refactor_every_step) { // Alg. 2 as printed: `_gesv` in the first iteration of every step
@@ -229,6 +238,7 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
     int *h_exec = reinterpret_cast<int *>(ctx->h_resid + 2 * OCI_RESID_CAP);
     while (it < max_iters && !conv_at) {
         const int k = (max_iters - it < check_every) ? max_iters - it : check_every;
+        NvtxRange batch(scheme == 0 ? "oci iteration batch" : "si iteration batch");
         OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
         // slot it + i > it looks at slot it + i - 1 on the device and skips itself once the rule held
         r = issue_batch(ctx, scheme, it, k, want_l2, true);
@@ -317,9 +327,24 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     ctx->opt_factor_kernel = 1;
     ctx->opt_factor_update = 1;
     ctx->opt_persistent = -1;
-    auto fail = [&](int code) { int lc = ctx->last_cuda; oci_destroy(ctx); (void)lc; return code; };
-    if (cudaGetDevice(&ctx->device) != cudaSuccess) return fail(OCI_E_CUDA);
-    device_limits(&ctx->num_sms, &ctx->max_smem_optin);
+    g_create_cuda_error = 0;
+    auto fail = [&](int code) { // keeps the CUDA error retrievable: oci_last_create_error()
+        if (code == OCI_E_CUDA) {
+            g_create_cuda_error = (int)cudaGetLastError();
+            if (g_create_cuda_error == 0) g_create_cuda_error = ctx->last_cuda ? ctx->last_cuda : (int)cudaErrorUnknown;
+        }
+        oci_destroy(ctx);
+        return code;
+    };
+    // the context lives on the device that owns the workspace, whatever device is current in the calling thread
+    {
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, workspace_dev) != cudaSuccess) return fail(OCI_E_CUDA);
+        if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) { oci_destroy(ctx); return -2; }
+        ctx->device = pa.device;
+    }
+    DeviceGuard guard(ctx->device);
+    device_limits(&ctx->num_sms, &ctx->max_smem_optin, ctx->device);
     const size_t need = carve(ctx, (unsigned char *)workspace_dev, p->J, p->N, p->G, ctx->num_sms, ctx->max_smem_optin);
     if (need > workspace_bytes) return fail(OCI_E_WORKSPACE);
     if (cudaHostAlloc((void **)&ctx->h_resid, sizeof(double) * (2 * OCI_RESID_CAP + 2), cudaHostAllocDefault) != cudaSuccess)
@@ -357,6 +382,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
 void oci_destroy(oci_ctx *ctx)
 {
     if (!ctx) return;
+    DeviceGuard guard(ctx->device);
     if (ctx->h_resid) cudaFreeHost(ctx->h_resid);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
@@ -377,10 +403,12 @@ const char *oci_strerror(int code)
 }
 
 int oci_last_cuda_error(const oci_ctx *ctx) { return ctx ? ctx->last_cuda : 0; }
+int oci_last_create_error(void) { return g_create_cuda_error; }
 
 int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!key) return -2;
     if (!strcmp(key, "iterate_kernel")) ctx->opt_iterate_kernel = (int)value;
     else if (!strcmp(key, "iterate_stages")) ctx->opt_stages = (int)value;
@@ -412,6 +440,7 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
 int oci_set_dt(oci_ctx *ctx, double dt)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!(dt > 0.0)) return -2;
     if (dt != ctx->dt) {
         ctx->dt = dt;
@@ -425,6 +454,7 @@ int oci_set_dt(oci_ctx *ctx, double dt)
 int oci_set_source(oci_ctx *ctx, const double *q_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     const size_t bytes = sizeof(double) * (size_t)ctx->J * ctx->G * 4;
     if (q_dev) OCI_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->q, q_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
     else OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->q, 0, bytes, ctx->stream));
@@ -435,6 +465,7 @@ int oci_set_source(oci_ctx *ctx, const double *q_dev)
 int oci_set_incident(oci_ctx *ctx, const double *left_dev, const double *right_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     const size_t bytes = sizeof(double) * (size_t)ctx->G * ctx->N * 2;
     if (left_dev) OCI_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->inc_left, left_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
     if (right_dev) OCI_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->inc_right, right_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -444,6 +475,7 @@ int oci_set_incident(oci_ctx *ctx, const double *left_dev, const double *right_d
 int oci_set_state(oci_ctx *ctx, const double *psi_edge_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!psi_edge_dev) return -2;
     const size_t bytes = sizeof(double) * (size_t)ctx->J * ctx->G * ctx->N * 2;
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->psi_prev, psi_edge_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -458,6 +490,7 @@ int oci_set_state(oci_ctx *ctx, const double *psi_edge_dev)
 int oci_get_state(oci_ctx *ctx, double *psi_edge_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!psi_edge_dev) return -2;
     const size_t bytes = sizeof(double) * (size_t)ctx->J * ctx->G * ctx->N * 2;
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(psi_edge_dev, ctx->psi_prev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -467,6 +500,7 @@ int oci_get_state(oci_ctx *ctx, double *psi_edge_dev)
 int oci_set_iterate(oci_ctx *ctx, const double *psi_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!psi_dev) return -2;
     const size_t bytes = sizeof(double) * (size_t)ctx->J * ctx->n;
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->psi[ctx->cur], psi_dev, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -477,7 +511,9 @@ int oci_set_iterate(oci_ctx *ctx, const double *psi_dev)
 int oci_factor(oci_ctx *ctx)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (ctx->factored) return 0;
+    NvtxRange range(ctx->opt_solve_mode == 1 ? "oci_factor (structured)" : "oci_factor (dense)");
     OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
     int r = ctx->opt_solve_mode == 1 ? launch_st_factor(ctx) : launch_factor(ctx);
     if (r < 0) return r;
@@ -494,24 +530,39 @@ int oci_factor(oci_ctx *ctx)
     return 0;
 }
 
-int oci_iterate(oci_ctx *ctx, int32_t n_iters) { return iterate_impl(ctx, 0, n_iters); }
-int si_iterate(oci_ctx *ctx, int32_t n_iters) { return iterate_impl(ctx, 1, n_iters); }
+int oci_iterate(oci_ctx *ctx, int32_t n_iters)
+{
+    if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
+    return iterate_impl(ctx, 0, n_iters);
+}
+int si_iterate(oci_ctx *ctx, int32_t n_iters)
+{
+    if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
+    return iterate_impl(ctx, 1, n_iters);
+}
 
 int oci_step(oci_ctx *ctx, double tol, int32_t max_iters, int32_t check_every, int32_t stop_rule, int32_t advance,
              int32_t *iters_out, double *resid_out)
 {
+    if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     return step_impl(ctx, 0, tol, max_iters, check_every, stop_rule, advance, iters_out, resid_out);
 }
 
 int si_step(oci_ctx *ctx, double tol, int32_t max_iters, int32_t check_every, int32_t stop_rule, int32_t advance,
             int32_t *iters_out, double *resid_out)
 {
+    if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     return step_impl(ctx, 1, tol, max_iters, check_every, stop_rule, advance, iters_out, resid_out);
 }
 
 int oci_advance(oci_ctx *ctx)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     int r = launch_advance(ctx);
     if (r < 0) return r;
     ctx->c_valid = false;
@@ -521,6 +572,7 @@ int oci_advance(oci_ctx *ctx)
 int oci_scalar_flux(oci_ctx *ctx, double *phi_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!phi_dev) return -2;
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(phi_dev, ctx->phi, sizeof(double) * (size_t)ctx->J * ctx->G * 4,
                                       cudaMemcpyDeviceToDevice, ctx->stream));
@@ -530,6 +582,7 @@ int oci_scalar_flux(oci_ctx *ctx, double *phi_dev)
 int oci_angular_flux(oci_ctx *ctx, double *psi_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!psi_dev) return -2;
     OCI_CUDA_TRY(ctx, cudaMemcpyAsync(psi_dev, ctx->psi[ctx->cur], sizeof(double) * (size_t)ctx->J * ctx->n,
                                       cudaMemcpyDeviceToDevice, ctx->stream));
@@ -539,6 +592,7 @@ int oci_angular_flux(oci_ctx *ctx, double *psi_dev)
 int oci_residual_history(oci_ctx *ctx, int32_t kind, double *host_out, int32_t cap, int32_t *n)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (kind != 0 && kind != 1) return -2;
     if (!n) return -5;
     const int len = ctx->hist_len;
@@ -558,6 +612,7 @@ int oci_step_host(oci_ctx *ctx, int32_t scheme, const double *q_host, double tol
                   double *phi_host)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (scheme != 0 && scheme != 1) return -2;
     const size_t bytes = sizeof(double) * (size_t)ctx->J * ctx->G * 4;
     if (q_host) {
@@ -576,6 +631,7 @@ int oci_step_host(oci_ctx *ctx, int32_t scheme, const double *q_host, double tol
 int oci_debug_get_matrix(oci_ctx *ctx, int32_t cell, double *A_host)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (cell < 0 || cell >= ctx->J) return -2;
     if (!A_host) return -3;
     int r = launch_assemble_one(ctx, cell, ctx->scratch);
@@ -589,6 +645,7 @@ int oci_debug_get_matrix(oci_ctx *ctx, int32_t cell, double *A_host)
 int oci_debug_get_factor_input(oci_ctx *ctx, int32_t cell, double *A_host)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (cell < 0 || cell >= ctx->J) return -2;
     if (!A_host) return -3;
     int r = launch_factor_input(ctx, cell, ctx->scratch);
@@ -603,6 +660,7 @@ int oci_debug_get_factor_input(oci_ctx *ctx, int32_t cell, double *A_host)
 int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (cell < 0 || cell >= ctx->J) return -2;
     if (!Ainv_host) return -3;
     if (!ctx->factored) return OCI_E_STATE;
@@ -620,6 +678,7 @@ int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host)
 int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (!c_dev) return -2;
     long long l = 0;
     int r = ensure_const_rhs(ctx, &l);
@@ -632,6 +691,7 @@ int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev)
 int oci_last_timing(oci_ctx *ctx, int32_t which, double *ms, int64_t *launches)
 {
     if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
     if (which < 0 || which > 2) return -2;
     if (ctx->last_ms[which] < 0.0) {
         // ev0/ev1 bracket the most recent iterate / step call; valid only if `which` was that call

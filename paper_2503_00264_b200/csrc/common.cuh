@@ -15,6 +15,15 @@
         }                                                         \
     } while (0)
 
+constexpr int OCI_SMEM_SLOTS = 48;
+enum { // one slot per kernel instantiation that needs more than 48 KB of dynamic shared memory
+    SLOT_WPC = 0,      // + 2 * (RPL index) + want_l2   (6 slots)
+    SLOT_STREAM = 6,   // + want_l2                     (2 slots)
+    SLOT_SWEEP = 8,    // + lanes index                 (3 slots)
+    SLOT_STP = 11,     // + ((GC index) * 2 + CT index) * 2 + want_l2   (20 slots)
+    SLOT_FACTOR = 32   // factor kernels
+};
+
 // ------------------------------------------------------------------------------------------------------------
 // Context. All device pointers are carved out of the caller's workspace (the library never cudaMallocs).
 // ------------------------------------------------------------------------------------------------------------
@@ -69,6 +78,9 @@ struct oci_ctx {
     bool factored, c_valid, si_valid, phi_valid;
     // options
     int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering;
+    // largest dynamic shared-memory size already granted (cudaFuncSetAttribute) to each kernel this context launches;
+    // kept per context (= per device), never in function-local statics
+    size_t smem_granted[OCI_SMEM_SLOTS];
     // timing
     cudaEvent_t ev0, ev1;
     double last_ms[3];
@@ -121,6 +133,30 @@ struct IterParams {
     int stages;   // matrix ring depth
     int chunk_doubles;
     int color, ncolors;   // structured path: cells j = ncolors * i + color (ncolors = 1: all cells)
+};
+
+// opt-in dynamic shared memory for `fn`, once per (context, kernel, size)
+static inline cudaError_t grant_smem(oci_ctx *ctx, int slot, const void *fn, size_t smem)
+{
+    if (ctx->smem_granted[slot] >= smem) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) ctx->smem_granted[slot] = smem;
+    return e;
+}
+
+// Every entry point of the C ABI works on the device the context was created on, whatever device is current in the
+// calling thread; the caller's current device is restored on return.
+struct DeviceGuard {
+    int prev;
+    bool switched;
+    explicit DeviceGuard(int dev) : prev(dev), switched(false)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
 };
 
 static inline ProblemView make_view(const oci_ctx *c)

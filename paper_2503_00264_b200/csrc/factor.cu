@@ -181,9 +181,9 @@ template <int NQ> struct FrShared {
     int rho[64 * NQ], rhoinv[64 * NQ];
 };
 
-template <int NQ>
+template <int NQ, bool DUMP>
 __global__ void __launch_bounds__(FR_THREADS, NQ == 1 ? 3 : (NQ == 2 ? 2 : 1))
-factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
+factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__restrict__ dumpA, int dump_cell)
 {
     constexpr int n = 64 * NQ, TR = 2 * NQ, NPANEL = n / FR_NB;
     extern __shared__ __align__(16) unsigned char fr_smem[];
@@ -201,7 +201,7 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
         else cluster.sync();
     };
 
-    for (int cell = cluster_id; cell < P.J; cell += n_clusters) {
+    for (int cell = DUMP ? dump_cell : cluster_id; cell < P.J; cell += n_clusters) {
         // ---- a1: assemble the tile, bit-identical to a_entry() (same operations in the same order)
         double a[TR][8];
         {
@@ -248,6 +248,14 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
                     }
                 }
             }
+        }
+        if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
+#pragma unroll
+            for (int rr = 0; rr < TR; ++rr)
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    dumpA[(size_t)(64 * (rr >> 1) + 2 * lane + (rr & 1)) * n + 64 * q + 8 * w + c] = a[rr][c];
+            return;
         }
         bool used_r = false; // row threadIdx.x (the row this thread holds during panel phases) was a pivot row
         bool singular = false;
@@ -426,213 +434,6 @@ factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info)
             double *col = out + (size_t)sh.rho[64 * q + 8 * w + c] * n;
 #pragma unroll
             for (int rr = 0; rr < TR; ++rr) col[ro[rr]] = a[rr][c];
-        }
-    }
-}
-
-// ============================================================================================================
-// n = 64: two warps per cell, the production a1 + a2 kernel of the headline configuration.
-// ============================================================================================================
-// Same blocked Gauss-Jordan as factor_reg_kernel, re-tiled so that MORE CELLS are in flight per SM: the owner's
-// panel phase is a serial, latency-bound instruction stream, so the throughput of the kernel is (cells in flight
-// per SM) / (length of that stream). Lane l of warp w holds the rows {2 l, 2 l + 1} of the columns
-// [32 w, 32 w + 32): 64 doubles per lane, 64 threads and ~17 KB of shared memory per cell, five cells per SM
-// (factor_reg_kernel<1>: three). Panel p (8 columns) belongs to warp p / 4, sub-tile p % 4 of its registers. Every
-// panel, both warps refresh a shadow copy of their tiles in shared memory; the panel is then eliminated by BOTH warps
-// with one row per lane (read from the shadow): per pivot step a warp-level arg-max, the two candidates exchanged
-// through shared memory (one CTA barrier per step), an 8-wide row update -- about 70 instructions per step and no
-// idle warp, against 160 for one warp holding two rows per lane. Z goes to shared memory, the eliminated panel back
-// to its owner's registers, and both warps apply the rank-8 update to their 32 columns.
-constexpr int W2_THREADS = 64;
-
-struct W2Shared {
-    double S[2][32][64];           // [warp][local column][row]: shadow copy of the warp's tile, refreshed every panel
-    double Z[FR_NB][64];           // [b][row]
-    double Pn[FR_NB][64];          // [c][row]: the eliminated panel on its way back to the owner's registers
-    PivotSlot slot[2][2];             // [step parity][warp]
-    int rho[64], rhoinv[64];
-};
-
-__global__ void __maxnreg__(200) factor_w2_kernel(ProblemView P, double *__restrict__ Minv, int *info)
-{
-    constexpr int n = 64, NPANEL = n / FR_NB;
-    constexpr unsigned FULL = 0xffffffffu;
-    extern __shared__ __align__(16) unsigned char w2_smem[];
-    W2Shared &sh = *reinterpret_cast<W2Shared *>(w2_smem);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int N = P.N, G = P.G;
-
-    for (int cell = blockIdx.x; cell < P.J; cell += gridDim.x) {
-        // ---- a1: assemble rows {2 lane, 2 lane + 1} x columns [32 w, 32 w + 32), bit-identical to a_entry().
-        // Register layout a[local column][row parity]: the two rows of a column are adjacent (16-byte stores).
-        double a[32][2];
-        {
-            const double dx = P.dx[cell];
-            const int p0 = (lane & 1) * 2;
-            const int bm = lane >> 1, m = bm % N, g = bm / N;
-            const double sig = P.sigma_t[(size_t)cell * G + g], mu = P.mu[m];
-            const double av = __dmul_rn(__dadd_rn(fabs(mu), __dmul_rn(dx, sig)), 0.5);
-            const double gam = __ddiv_rn(dx, __dmul_rn(P.v[g], P.dt));
-            const double h = __dmul_rn(mu, 0.5), hg = __dmul_rn(gam, 0.5), ga = __dadd_rn(gam, av);
-#pragma unroll
-            for (int cb = 0; cb < 8; ++cb) { // column block (g', m') = 8 w + cb
-                const int bmc = 8 * w + cb;
-                const double K = P.transfer[((size_t)cell * G + g) * G + bmc / N];
-                const double Kw = __dmul_rn(__dmul_rn(__dmul_rn(dx, K), 0.25), P.w[bmc % N]);
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int p = p0 + e;
-#pragma unroll
-                    for (int pp = 0; pp < 4; ++pp) {
-                        double val = 0.0;
-                        if (bm == bmc) { // Eq. 8b
-                            const int d = pp - p;
-                            if (d == 0) val = p < 2 ? av : ga;
-                            else if (p == 0 && pp == 1) val = h;
-                            else if (p == 1 && pp == 0) val = -h;
-                            else if (p == 2 && pp == 3) val = h;
-                            else if (p == 3 && pp == 2) val = -h;
-                            else if (d == 2) val = hg;
-                            else if (d == -2) val = -gam;
-                        }
-                        if (p == pp) val = __dsub_rn(val, Kw);
-                        a[4 * cb + pp][e] = val;
-                    }
-                }
-            }
-        }
-        bool used_r = false;   // row 32 w + lane (the row this lane holds during the panel phases) was a pivot row
-        bool singular = false;
-        double2 *Sw = reinterpret_cast<double2 *>(&sh.S[w][0][0]); // [local column][32 lanes] of double2
-        const int r = 32 * w + lane;
-
-        for (int pnl = 0; pnl < NPANEL; ++pnl) {
-            const int wo = pnl >> 2, st = pnl & 3;
-            const bool owner = wo == w;
-            // ---- shadow copy of this warp's tile: the panel phase reads the panel from it row by row, phase U its pivot
-            // rows (conflict-free 16-byte stores)
-#pragma unroll
-            for (int c = 0; c < 32; ++c) Sw[c * 32 + lane] = make_double2(a[c][0], a[c][1]);
-            __syncthreads();
-
-            // ================= phase P: both warps eliminate the 64 x 8 panel, ONE ROW PER LANE =================
-            double t[FR_NB];
-#pragma unroll
-            for (int c = 0; c < FR_NB; ++c) t[c] = sh.S[wo][8 * st + c][r];
-            int Rl[FR_NB];
-            bool bad = false;
-#pragma unroll
-            for (int b = 0; b < FR_NB; ++b) {
-                // local (warp) arg-max over the unused rows: first row of maximal |entry|
-                const unsigned long long key = used_r ? 0ull : (unsigned long long)__double_as_longlong(fabs(t[b]));
-                const unsigned khi = (unsigned)(key >> 32);
-                const unsigned mhi = __reduce_max_sync(FULL, khi);
-                // in the shadow of the reduction: this lane's row scaled by 1 / its candidate
-                const double linv = rcp_nr(t[b]);
-                double scl[FR_NB];
-#pragma unroll
-                for (int c = 0; c < FR_NB; ++c) scl[c] = (c == b) ? linv : t[c] * linv;
-                bool cand = !used_r && khi == mhi;
-                const unsigned ball = __ballot_sync(FULL, cand);
-                int src;
-                if (__popc(ball) == 1) {
-                    src = __ffs(ball) - 1;
-                } else { // ties in the high word (or no unused row in this warp): low words, then the lowest row
-                    const unsigned klo = (unsigned)key;
-                    const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
-                    cand = cand && klo == mlo;
-                    const unsigned b2 = __ballot_sync(FULL, cand);
-                    src = b2 ? __ffs(b2) - 1 : 0;
-                }
-                PivotSlot *mys = &sh.slot[b & 1][w];
-                if (lane == src) {
-#pragma unroll
-                    for (int c = 0; c < FR_NB / 2; ++c)
-                        reinterpret_cast<double2 *>(mys->row)[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
-                    mys->key = key;
-                    mys->lane = lane;
-                }
-                __syncthreads(); // the two candidates of this step are visible (two slot buffers alternate)
-                const unsigned long long k0 = sh.slot[b & 1][0].key, k1 = sh.slot[b & 1][1].key;
-                const int gw = k1 > k0 ? 1 : 0; // a tie goes to warp 0: the lower row
-                const unsigned long long kmax = gw ? k1 : k0;
-                if ((unsigned)(kmax >> 32) == 0u || (unsigned)(kmax >> 32) >= 0x7ff00000u) bad = true; // zero / denormal / inf / NaN
-                const PivotSlot *win = &sh.slot[b & 1][gw];
-                const int lw = win->lane;
-                Rl[b] = 32 * gw + lw;
-                double sp[FR_NB];
-#pragma unroll
-                for (int c = 0; c < FR_NB / 2; ++c) {
-                    const double2 v = reinterpret_cast<const double2 *>(win->row)[c];
-                    sp[2 * c] = v.x;
-                    sp[2 * c + 1] = v.y;
-                }
-                const bool is_p = gw == w && lane == lw;
-                const double f = t[b];
-#pragma unroll
-                for (int c = 0; c < FR_NB; ++c) { // the pivot row becomes itself / pivot (= scl, computed above)
-                    const double upd = (c == b) ? -f * sp[b] : fma(-f, sp[c], t[c]);
-                    t[c] = is_p ? scl[c] : upd;
-                }
-                if (is_p) used_r = true;
-                if (threadIdx.x == b) { sh.rho[FR_NB * pnl + b] = Rl[b]; sh.rhoinv[Rl[b]] = FR_NB * pnl + b; }
-            }
-            // ---- publish Z = T[:, R] - I[:, R] and the eliminated panel; the owner's shadow of the panel columns becomes 0
-            // so that phase U leaves them alone
-#pragma unroll
-            for (int b = 0; b < FR_NB; ++b) {
-                sh.Z[b][r] = t[b] - (Rl[b] == r ? 1.0 : 0.0);
-                sh.Pn[b][r] = t[b];
-            }
-            if (owner) {
-#pragma unroll
-                for (int c = 0; c < FR_NB; ++c) Sw[(8 * st + c) * 32 + lane] = make_double2(0.0, 0.0);
-            }
-            __syncthreads();
-            if (bad) { singular = true; break; } // uniform across the CTA
-            if (owner) { // the panel's own columns now hold T e_r
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (k == st) {
-#pragma unroll
-                        for (int c = 0; c < FR_NB; ++c) {
-                            const double2 v = *reinterpret_cast<const double2 *>(&sh.Pn[c][2 * lane]);
-                            a[8 * k + c][0] = v.x;
-                            a[8 * k + c][1] = v.y;
-                        }
-                    }
-            }
-
-            // ---- phase U: rank-8 update  a[:, c] += Z[:, b] * W_old[r_b, c]  of this lane's 2 x 32 tile
-#pragma unroll
-            for (int b = 0; b < FR_NB; ++b) {
-                const double2 z = *reinterpret_cast<const double2 *>(&sh.Z[b][2 * lane]);
-                const double *row = &sh.S[w][0][Rl[b]]; // W_old[r_b, local column c] at row[64 c] (uniform address)
-#pragma unroll
-                for (int c = 0; c < 32; ++c) {
-                    const double rv = row[64 * c];
-                    a[c][0] = fma(z.x, rv, a[c][0]);
-                    a[c][1] = fma(z.y, rv, a[c][1]);
-                }
-            }
-            __syncwarp(); // every lane is done with the shadow before the next panel overwrites it
-        }
-
-        __syncthreads(); // rho / rhoinv complete and visible
-        double *out = Minv + (size_t)cell * n * n;
-        if (singular) {
-            if (threadIdx.x == 0) atomicMin(info, cell + 1);
-            for (int e = threadIdx.x; e < n * n; e += W2_THREADS) out[e] = 0.0;
-            __syncthreads();
-            continue;
-        }
-        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]
-        const int ro0 = sh.rhoinv[2 * lane], ro1 = sh.rhoinv[2 * lane + 1];
-#pragma unroll
-        for (int c = 0; c < 32; ++c) {
-            double *col = out + (size_t)sh.rho[32 * w + c] * n;
-            col[ro0] = a[c][0];
-            col[ro1] = a[c][1];
         }
     }
 }
@@ -1232,13 +1033,13 @@ size_t factor_scratch_bytes(int n, int num_sms, int max_smem_optin)
     return one * (size_t)num_sms * 4;
 }
 
-template <int NQ> static int launch_factor_reg(oci_ctx *ctx, const ProblemView &P)
+template <int NQ, bool DUMP> static int launch_factor_reg_t(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.blockDim = dim3(FR_THREADS, 1, 1);
     cfg.dynamicSmemBytes = sizeof(FrShared<NQ>);
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_reg_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_reg_kernel<NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)sizeof(FrShared<NQ>)));
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
@@ -1248,21 +1049,42 @@ template <int NQ> static int launch_factor_reg(oci_ctx *ctx, const ProblemView &
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = NQ > 1 ? 1 : 0;
-    int n_clusters = 0;
-    if (NQ > 1) {
-        cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_reg_kernel<NQ>, &cfg));
-    } else {
-        int per_sm = 0;
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_reg_kernel<NQ>, FR_THREADS,
-                                                                        sizeof(FrShared<NQ>)));
-        n_clusters = per_sm * ctx->num_sms;
+    int n_clusters = 1;
+    if (!DUMP) {
+        if (NQ > 1) {
+            cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
+            OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_reg_kernel<NQ, DUMP>, &cfg));
+        } else {
+            int per_sm = 0;
+            OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_reg_kernel<NQ, DUMP>, FR_THREADS,
+                                                                            sizeof(FrShared<NQ>)));
+            n_clusters = per_sm * ctx->num_sms;
+        }
+        if (n_clusters < 1) n_clusters = 1;
+        if (n_clusters > ctx->J) n_clusters = ctx->J;
     }
-    if (n_clusters < 1) n_clusters = 1;
-    if (n_clusters > ctx->J) n_clusters = ctx->J;
     cfg.gridDim = dim3(NQ * n_clusters, 1, 1);
-    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_reg_kernel<NQ>, P, ctx->Minv, ctx->info));
+    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_reg_kernel<NQ, DUMP>, P, ctx->Minv, ctx->info, dumpA, dump_cell));
     return 1;
+}
+
+// dumpA != nullptr: only assemble `dump_cell` and write the tile there
+static int launch_factor_reg_n(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
+{
+    if (dumpA) {
+        switch (ctx->n / 64) {
+        case 1: return launch_factor_reg_t<1, true>(ctx, P, dumpA, dump_cell);
+        case 2: return launch_factor_reg_t<2, true>(ctx, P, dumpA, dump_cell);
+        case 3: return launch_factor_reg_t<3, true>(ctx, P, dumpA, dump_cell);
+        default: return launch_factor_reg_t<4, true>(ctx, P, dumpA, dump_cell);
+        }
+    }
+    switch (ctx->n / 64) {
+    case 1: return launch_factor_reg_t<1, false>(ctx, P, nullptr, 0);
+    case 2: return launch_factor_reg_t<2, false>(ctx, P, nullptr, 0);
+    case 3: return launch_factor_reg_t<3, false>(ctx, P, nullptr, 0);
+    default: return launch_factor_reg_t<4, false>(ctx, P, nullptr, 0);
+    }
 }
 
 // n = 64, one warp per cell (factor_wc_kernel). dumpA != nullptr: only assemble `dump_cell` and write the tile there.
@@ -1302,25 +1124,8 @@ int launch_factor(oci_ctx *ctx)
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream)); // 0x7f7f7f7f = "none"
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && n == 64) return launch_factor_wc(ctx, P, nullptr, 0);
-    if (ctx->opt_factor_kernel == 3 && n == 64) { // the register-resident two-warp kernel of round 1 (kept for the A/B)
-        int per_sm = 0;
-        const size_t smem = sizeof(W2Shared);
-        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_w2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_w2_kernel, W2_THREADS, smem));
-        int grid = (per_sm < 1 ? 1 : per_sm) * ctx->num_sms;
-        if (grid > ctx->J) grid = ctx->J;
-        factor_w2_kernel<<<grid, W2_THREADS, smem, ctx->stream>>>(P, ctx->Minv, ctx->info);
-        OCI_CUDA_TRY(ctx, cudaGetLastError());
-        return 1;
-    }
-    if (ctx->opt_factor_kernel >= 1 && n % 64 == 0 && n <= 256) { // 2: the 8-warp kernel also for n = 64
-        switch (n / 64) {
-        case 1: return launch_factor_reg<1>(ctx, P);
-        case 2: return launch_factor_reg<2>(ctx, P);
-        case 3: return launch_factor_reg<3>(ctx, P);
-        default: return launch_factor_reg<4>(ctx, P);
-        }
-    }
+    if (ctx->opt_factor_kernel >= 1 && n % 64 == 0 && n <= 256) // 2: the 8-warp kernel also for n = 64
+        return launch_factor_reg_n(ctx, P, nullptr, 0);
     const bool global_w = factor_smem_bytes(n, false) > (size_t)ctx->max_smem_optin;
     const size_t smem = factor_smem_bytes(n, global_w);
     int grid;
@@ -1351,6 +1156,7 @@ int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor)
     ProblemView P = make_view(ctx);
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && ctx->n == 64)
         return launch_factor_wc(ctx, P, A_dev_rowmajor, cell);
+    if (ctx->opt_factor_kernel >= 1 && ctx->n % 64 == 0 && ctx->n <= 256) return launch_factor_reg_n(ctx, P, A_dev_rowmajor, cell);
     return 0;
 }
 

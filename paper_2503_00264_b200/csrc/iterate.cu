@@ -603,12 +603,8 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
         if (grid > (ctx->J + WPC_WARPS - 1) / WPC_WARPS) grid = (ctx->J + WPC_WARPS - 1) / WPC_WARPS;
 #define OCI_WPC_LAUNCH(RPL_, L2_)                                                                                  \
     do {                                                                                                           \
-        static size_t attr = 0;                                                                                    \
-        if (attr < smem) {                                                                                         \
-            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(oci_iterate_wpc_kernel<RPL_, L2_>,                               \
-                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
-            attr = smem;                                                                                           \
-        }                                                                                                          \
+        OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_WPC + (RPL_ == 2 ? 0 : (RPL_ == 4 ? 2 : 4)) + (L2_ ? 1 : 0),         \
+                                     (const void *)oci_iterate_wpc_kernel<RPL_, L2_>, smem));                      \
         oci_iterate_wpc_kernel<RPL_, L2_><<<grid, WPC_THREADS, smem, ctx->stream>>>(P);                             \
     } while (0)
         if (n == 64) { if (want_l2) OCI_WPC_LAUNCH(2, true); else OCI_WPC_LAUNCH(2, false); }
@@ -627,16 +623,9 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
         P.cpb = pl.cpb; P.S = pl.S; P.cw = pl.cw; P.nch = pl.nch; P.stages = pl.stages;
         P.chunk_doubles = pl.chunk_doubles;
         P.n_items = (ctx->J + pl.cpb - 1) / pl.cpb;
-        static size_t attr_set[2] = {0, 0};
-        if (attr_set[want_l2] < pl.smem) {
-            if (want_l2)
-                OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(oci_iterate_stream_kernel<true>,
-                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-            else
-                OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(oci_iterate_stream_kernel<false>,
-                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-            attr_set[want_l2] = pl.smem;
-        }
+        OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_STREAM + (want_l2 ? 1 : 0),
+                                     want_l2 ? (const void *)oci_iterate_stream_kernel<true>
+                                             : (const void *)oci_iterate_stream_kernel<false>, pl.smem));
         if (want_l2) oci_iterate_stream_kernel<true><<<pl.grid, ITER_THREADS, pl.smem, ctx->stream>>>(P);
         else oci_iterate_stream_kernel<false><<<pl.grid, ITER_THREADS, pl.smem, ctx->stream>>>(P);
     }

@@ -495,12 +495,8 @@ int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_pr
 #define OCI_SWEEP(LPC_)                                                                                            \
     do {                                                                                                           \
         const size_t smem = sizeof(double) * sw_stages(LPC_) * TC * LPC_ * 8 + 3 * sw_stages(LPC_) * sizeof(uint64_t);         \
-        static bool attr_set = false;                                                                              \
-        if (!attr_set) {                                                                                           \
-            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(si_sweep_kernel<LPC_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                                   (int)smem));                                                    \
-            attr_set = true;                                                                                       \
-        }                                                                                                          \
+        OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_SWEEP + (LPC_ == 4 ? 0 : (LPC_ == 8 ? 1 : 2)),                       \
+                                     (const void *)si_sweep_kernel<LPC_>, smem));                                  \
         si_sweep_kernel<LPC_><<<sweep_grid, SW_THREADS, smem, ctx->stream>>>(                                       \
             stop, ctx->J, ctx->N, ctx->G, ctx->bc_left, ctx->bc_right, ctx->mu, ctx->si_T2sw, ctx->si_bsw, psi,      \
             ctx->inc_left, ctx->inc_right, ctx->si_in);                                                            \

@@ -652,12 +652,9 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
             if (grid > (ctx->J + CPB - 1) / CPB) grid = (ctx->J + CPB - 1) / CPB;
 #define OCI_STP_LAUNCH(L2_, GC_, CT_)                                                                              \
     do {                                                                                                           \
-        static size_t attr = 0;                                                                                    \
-        if (attr < smem) {                                                                                         \
-            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(st_iterate_pipe_kernel<L2_, GC_, CT_>,                          \
-                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
-            attr = smem;                                                                                           \
-        }                                                                                                          \
+        OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_STP + (((GC_ == 0 ? 0 : (GC_ == 1 ? 1 : (GC_ == 2 ? 2 : (GC_ == 4 ? 3 : 4)))) * 2 + \
+                                                      (CT_ == 128 ? 0 : 1)) * 2 + (L2_ ? 1 : 0)),                  \
+                                     (const void *)st_iterate_pipe_kernel<L2_, GC_, CT_>, smem));                  \
         st_iterate_pipe_kernel<L2_, GC_, CT_><<<grid, CT_ + 32, smem, ctx->stream>>>(P, S, stages);                \
     } while (0)
 #define OCI_STP_G(GC_)                                                                                             \

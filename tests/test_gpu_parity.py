@@ -31,7 +31,7 @@ def rel(a, b):
 
 
 SMALL_CASES = [
-    # seed, J, N, G, bc_left, bc_right   (n = 4NG: 8, 16, 24, 32, 48, 64, 96, 128, 160, 256; ragged J everywhere)
+    # seed, J, N, G, bc_left, bc_right   (n = 4NG: 8, 16, 24, 32, 48, 64, 96, 128, 160, 200, 256; ragged J everywhere)
     (1, 5, 2, 1, 0, 0),
     (2, 37, 4, 1, 0, 0),
     (3, 19, 2, 3, 1, 0),
@@ -44,6 +44,9 @@ SMALL_CASES = [
     (10, 11, 8, 8, 1, 0),
     (11, 1, 4, 2, 0, 0),      # a single cell: both neighbours are boundaries
     (12, 2, 2, 1, 1, 1),
+    (18, 300, 2, 1, 0, 2),    # S2 with J G > 64: 128 (j, g) pairs per block of si_finish_kernel (the round-1 bug)
+    (19, 200, 2, 3, 1, 0),    # S2, three groups
+    (20, 6, 10, 5, 0, 0),     # n = 200: not a multiple of 64 and too large for shared memory (global-scratch factor path)
 ]
 
 

@@ -128,3 +128,76 @@ def test_redblack_reaches_the_same_fixed_point_in_about_half_the_iterations():
     np.testing.assert_allclose(rb.psi, exact, rtol=0, atol=1e-10 * scale + 1e-12)
     np.testing.assert_allclose(jac.psi, exact, rtol=0, atol=1e-10 * scale + 1e-12)
     assert 0.4 * it_j <= it_r <= 0.65 * it_j, (it_j, it_r)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# The stopping arithmetic itself (Eq. 12-13; Alg. 2; Eq. 46 for SI), pinned hard:
+# the tested quantity of every iteration and the iteration at which the loop stops are re-evaluated in numpy from
+# iterates obtained one iteration at a time, never from the loop under test.
+# ---------------------------------------------------------------------------------------------------------------
+def _stop_index(e, tol, rule):
+    """First 0-based l at which the rule holds for the tested quantities e[0], e[1], ...: rule 0: e_l < tol; rule 1:
+    e_l < tol (1 - e_l / e_{l-1}), tested from l >= 1 (Alg. 2 computes e only in its else-branch)."""
+    for l in range(len(e)):
+        if rule == 0 and e[l] < tol:
+            return l
+        if rule == 1 and l >= 1 and e[l] < tol * (1.0 - e[l] / e[l - 1]):
+            return l
+    return None
+
+
+@pytest.mark.parametrize("scheme", ["oci", "si"])
+@pytest.mark.parametrize("rule", [0, 1])
+def test_stop_rules_tested_quantity_and_stop_iteration(scheme, rule):
+    p = W.random_problem(91, J=23, N=4, G=2, bc_left=W.BC_REFLECTIVE, bc_right=W.BC_PRESCRIBED, dt=0.4, c_max=0.9)
+    tol = 1e-7
+    # the loop under test
+    o = oracle.Oracle(p)
+    it, hist = (o.oci_step if scheme == "oci" else o.si_step)(tol=tol, rule=rule, advance=False)
+    # the same iterates, one iteration at a time, norms taken by numpy
+    s = oracle.Oracle(p)
+    if scheme == "oci":
+        s.factor()
+        s.const_rhs()
+    e = []
+    for l in range(it + 3):
+        psi_old, phi_old = s.psi.copy(), s.phi.copy()
+        s.oci_iterate(1) if scheme == "oci" else s.si_iterate(1)
+        if rule == 0:
+            e.append(np.max(np.abs(s.phi - phi_old)))                       # BASELINE.json: |dphi|_inf
+        elif scheme == "oci":
+            e.append(np.linalg.norm((s.psi - psi_old).reshape(-1)))         # Eq. 12: ||Psi^(l+1) - Psi^(l)||_2
+        else:
+            e.append(np.linalg.norm((s.phi - phi_old).reshape(-1)))         # Eq. 46: ||phi^(l+1) - phi^(l)||_2
+    e = np.array(e)
+    np.testing.assert_allclose(hist, e[:it], rtol=1e-12, atol=0)
+    stop = _stop_index(e, tol, rule)
+    assert stop is not None and it == stop + 1, (it, stop)
+    if rule == 1:
+        # a max-norm in place of the 2-norm, or a test that starts at l = 0, would stop elsewhere on this problem
+        e_inf = []
+        s2 = oracle.Oracle(p)
+        if scheme == "oci":
+            s2.factor()
+            s2.const_rhs()
+        for l in range(it + 3):
+            old = (s2.psi if scheme == "oci" else s2.phi).copy()
+            s2.oci_iterate(1) if scheme == "oci" else s2.si_iterate(1)
+            e_inf.append(np.max(np.abs((s2.psi if scheme == "oci" else s2.phi) - old)))
+        assert _stop_index(np.array(e_inf), tol, 1) != stop
+        assert hist[0] > tol                                                 # l = 0 is recorded but never tested
+
+
+def test_rule1_counts_on_config2_first_step():
+    """SURVEY 8(c) H1, re-derived here: config 2 at dt = 1, J = 1024, first step. Rule 0 (|dphi|_inf < 1e-8) stops after
+    725 iterations with a true error of ~5e-7; the paper's rule 1 (eps = 1e-8) needs 1145 (rho_e ~ 0.974) and ends
+    ~1e-10 from the fixed point: the (1 - rho_e) factor does what PAPER.md:441-442 says."""
+    p = W.config2(dt=1.0)
+    o0, o1, ref = oracle.Oracle(p), oracle.Oracle(p), oracle.Oracle(p)
+    it0, _ = o0.oci_step(tol=1e-8, rule=0, advance=False)
+    it1, h1 = o1.oci_step(tol=1e-8, rule=1, advance=False)
+    assert (it0, it1) == (725, 1145)
+    assert abs(h1[-1] / h1[-2] - 0.974) < 2e-3
+    ref.oci_step(tol=1e-14, max_iters=200000, advance=False)
+    err0, err1 = np.abs(o0.phi - ref.phi).max(), np.abs(o1.phi - ref.phi).max()
+    assert 2e-7 < err0 < 1e-6 and err1 < 5e-10
