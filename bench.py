@@ -46,13 +46,15 @@ CHECK_EVERY = 8
 MAX_ITERS = 4000
 METRIC = "oci_cell_solves_per_s"
 UNIT = "cell-solves/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one oci_iterate_wpc_kernel<2,0> launch on this workload, from the
-# `ncu --set full` capture summarised in profiles/r01_c_ncu_full.md (2.214779 GB read + 38.01 MB written).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 2252789624
-# same for one factor launch (factor_w2_kernel, profiles/r01_e_factor.md)
-NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH = 2090512639
-# same for one st_iterate_pipe_kernel<0,1> launch (profiles/r01_d_ncu_full.md): 213.30 MB read + 21.86 MB written
-NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH = 235150848
+# `traffic` (dram__bytes_read.sum + dram__bytes_write.sum per launch, from `ncu --set full`) is read from
+# profiles/r02_kernel_traffic.csv, which records for every capture the hash of the kernel's source files; a value is
+# printed only if that hash equals the hash of the sources this run was built from (ncu_traffic() below).
+TRAFFIC_FILE = "profiles/r02_kernel_traffic.csv"
+KERNEL_SOURCES = {   # kernel -> the files (under paper_2503_00264_b200/csrc/) its code lives in
+    "oci_iterate_wpc_kernel": ["iterate.cu", "common.cuh"],
+    "factor_wc2_kernel": ["factor.cu", "common.cuh"],
+    "st_iterate_pipe_kernel": ["structured.cu", "common.cuh"],
+}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
                                                     # .sum.peak_sustained = 64 per SM) x 2 flop x clocks.max.sm
 
@@ -66,6 +68,33 @@ def measured_peaks():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def source_hash(kernel: str) -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES[kernel]:
+        h.update((ROOT / "paper_2503_00264_b200" / "csrc" / name).read_bytes())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """(bytes per launch or None, note). None unless the capture on file was taken with exactly these kernel sources."""
+    f = ROOT / TRAFFIC_FILE
+    if not f.exists():
+        return None, f"{TRAFFIC_FILE} missing"
+    want = source_hash(kernel)
+    stale = None
+    for line in f.read_text().splitlines():
+        c = [x.strip() for x in line.split(",")]
+        if len(c) < 6 or c[0] != kernel or c[2] != workload:
+            continue
+        if c[1] == want:
+            return int(c[3]) + int(c[4]), f"{TRAFFIC_FILE}: {c[5]} (source hash {want})"
+        stale = c[1]
+    if stale:
+        return None, f"capture on file is of other sources (hash {stale}, built from {want}): not quoted"
+    return None, f"no capture of {kernel} on {workload} in {TRAFFIC_FILE}"
 
 
 def structured_bytes_per_cell_solve(n: int, G: int) -> int:
@@ -331,29 +360,38 @@ def run_ours(args):
     launch_ms = kernel_ms_total / max(iters_total, 1)
     alg_bytes = algorithmic_bytes_per_cell_solve(n, G) * J
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+    wl = "config5"
+    tr, tr_note = ncu_traffic("oci_iterate_wpc_kernel", wl)
     roofline = {"bound": "hbm", "kernel": "oci_iterate_wpc_kernel<2,0>", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": tr, "traffic_source": tr_note,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": launch_ms,
                 "kernel_share_of_step": kernel_ms_total / ms_total}
     factor_ms = statistics.mean(x for d in per_dt.values() for x in d["factor_ms"])
-    factor_tf = 2.0 * n ** 3 * J / (factor_ms * 1e-3) / 1e12
-    roofline_factor = {"bound": "alu", "kernel": "factor_w2_kernel", "achieved": factor_tf, "peak": FP64_PEAK_TFLOPS,
+    exec_flops, alg_flops = 2.0 * n ** 3 * J, (2.0 / 3.0) * n ** 3 * J
+    factor_tf = exec_flops / (factor_ms * 1e-3) / 1e12
+    tr, tr_note = ncu_traffic("factor_wc2_kernel", wl)
+    roofline_factor = {"bound": "alu", "kernel": "factor_wc2_kernel", "achieved": factor_tf, "peak": FP64_PEAK_TFLOPS,
                        "unit": "TFLOP/s", "frac": factor_tf / FP64_PEAK_TFLOPS,
-                       "traffic": NCU_FACTOR_TRAFFIC_BYTES_PER_LAUNCH,
-                       "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md section 7)",
-                       "flops_per_launch": 2.0 * n ** 3 * J, "avg_launch_ms": factor_ms,
-                       "kernel_share_of_step": factor_ms * K / ms_total}
+                       "frac_algorithmic": alg_flops / (factor_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                       "executed_flops": exec_flops, "algorithmic_flops": alg_flops,
+                       "flops_note": "executed = 2 n^3 per cell (Gauss-Jordan with partial pivoting carried to the inverse, "
+                                     "what the kernel does); algorithmic = (2/3) n^3 per cell (the LU of SURVEY 8(d))",
+                       "traffic": tr, "traffic_source": tr_note,
+                       "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz (DESIGN.md section 7); DMMA "
+                                      "reaches the same 64 FMA/clk/SM (profiles/r02_fp64_pipe.md)",
+                       "avg_launch_ms": factor_ms, "kernel_share_of_step": factor_ms * K / ms_total}
 
     st_launch_ms = st_kernel_ms / max(st_iters, 1)
     st_bytes = structured_bytes_per_cell_solve(n, G) * J
     st_achieved = st_bytes / (st_launch_ms * 1e-3) / 1e9
+    st_tr, st_tr_note = ncu_traffic("st_iterate_pipe_kernel", wl)
     structured = {
         "what": "SURVEY 8(f) row f1: structured cell solve A_j = D - U V^T (solve_mode = 1), same steps, same stop rule",
         "value": whole_job_value(world, J, st_iters, st_ms_total), "unit": UNIT, "ms_per_step": st_ms_total / K,
         "iterations_total": st_iters, "factor_ms": statistics.mean(st_factor_ms),
         "max_abs_phi_minus_dense_path": st_diff,
         "roofline": {"bound": "hbm", "kernel": "st_iterate_pipe_kernel<0,1>", "achieved": st_achieved, "peak": peak, "unit": "GB/s",
-                     "frac": st_achieved / peak, "traffic": NCU_STRUCTURED_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
+                     "frac": st_achieved / peak, "traffic": st_tr, "traffic_source": st_tr_note, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": st_bytes, "avg_launch_ms": st_launch_ms,
                      "kernel_share_of_step": st_kernel_ms / st_ms_total},
     }
@@ -371,6 +409,12 @@ def run_ours(args):
                "sample": f"first {sample.J} of {J} cells of config 5, {passes} pass(es) of one converged time step at each "
                          f"dt of {SWEEP} (factor + iterate + advance), {secs:.1f} s",
                "iters": [d["iters"] for d in cpu_dt]}
+
+    per_config = true_error = as_specified = None
+    if world == 1 and not args.quick:
+        per_config = run_per_config(f"cuda:{local}", peak)
+        true_error = run_true_error(p, f"cuda:{local}")
+        as_specified = run_as_specified(p, f"cuda:{local}", args.no_si)
 
     table = []
     for dt in SWEEP:
@@ -400,12 +444,127 @@ def run_ours(args):
         "structured": structured,
         "cpu_baseline": cpu,
         "oci_vs_si": table,
+        "as_specified": as_specified,
+        "true_error": true_error,
+        "per_config": per_config,
         "max_abs_phi_oci_minus_si": diff,
         "iterations_total": iters_total,
     }
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Legs reported beside the headline (none of them is part of `value`)
+# ---------------------------------------------------------------------------------------------------------------
+def empty_launch_us(solver, torch, n=200):
+    """Device time per launch of an empty kernel in a stream of back-to-back launches (the floor of one iteration)."""
+    solver.debug_empty_launches(20)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    solver.debug_empty_launches(n)
+    e1.record()
+    torch.cuda.synchronize()
+    return 1e3 * e0.elapsed_time(e1) / n
+
+
+def run_per_config(device, peak):
+    """BASELINE.json configs 1-4 (+ variant 4b), each run as configured for a few steps on the dense path (the
+    structured path beside it): iterations OCI vs SI, ms per converged step, us per iteration, factor ms, and for the
+    HBM-bound ones (3, 4) the roofline fraction of the iterate kernel; for the L2-resident ones (1, 2) the iteration
+    time against the measured empty-launch floor (no roofline fraction is meaningful there)."""
+    import torch
+    from paper_2503_00264_b200 import OCISolver
+    cases = [("config1", W.config1(), 0.1, 5), ("config2@dt=1", W.config2(dt=1.0), 1.0, 3),
+             ("config2@dt=0.1", W.config2(dt=0.1), 0.1, 5), ("config2@dt=0.01", W.config2(dt=0.01), 0.01, 5),
+             ("config3", W.config3(), 1e-8, 5), ("config4", W.config4(), 1e-3, 5),
+             ("config4b(v=1000)", W.config4(v=1000.0), 1e-3, 3)]
+    out = []
+    floor = None
+    for name, p, dt, steps in cases:
+        row = {"config": name, "J": p.J, "N": p.N, "G": p.G, "n": p.n, "dt": dt, "steps": steps}
+        for key, scheme, opts in (("oci_dense", 0, {}), ("oci_structured", 0, {"solve_mode": 1}), ("si", 1, {})):
+            sol = OCISolver(p, dt=dt, device=device, options=opts)
+            if floor is None:
+                floor = empty_launch_us(sol, torch)
+            if scheme == 0:
+                sol.factor()                       # warm-up of the factor kernel; re-done (timed) below
+                sol.set_dt(dt * (1 + 1e-12)); sol.factor()
+                row[key + "_factor_ms"] = sol.last_timing(0)[0]
+            iters, ms, kms = [], [], []
+            for st in range(steps):
+                sol.set_source(p.source_at_step(st))
+                torch.cuda.synchronize(); t = time.perf_counter()
+                it, conv, _ = (sol.step if scheme == 0 else sol.si_step)(tol=p.tol, max_iters=20000, check_every=CHECK_EVERY)
+                ms.append((time.perf_counter() - t) * 1e3)
+                iters.append(it)
+                kms.append(sol.last_timing(1 if scheme == 0 else 2)[0])
+            row[key + "_iters"] = iters
+            row[key + "_ms_per_step"] = statistics.mean(ms)
+            row[key + "_us_per_iteration"] = 1e3 * sum(kms) / max(sum(iters), 1)
+            if key == "oci_dense":
+                us = row[key + "_us_per_iteration"]
+                if p.J * p.n * p.n * 8 > (126 << 20):     # factors exceed the L2: HBM roofline
+                    gbs = algorithmic_bytes_per_cell_solve(p.n, p.G) * p.J / (us * 1e-6) / 1e9
+                    row["oci_dense_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak}
+                else:
+                    row["oci_dense_iteration_over_launch_floor"] = us / floor
+                fl = 2.0 * p.n ** 3 * p.J
+                row["oci_dense_factor_tflops_executed"] = fl / (row[key + "_factor_ms"] * 1e-3) / 1e12
+                row["oci_dense_factor_frac_of_fp64_peak_executed"] = row["oci_dense_factor_tflops_executed"] / FP64_PEAK_TFLOPS
+                row["oci_dense_factor_frac_of_fp64_peak_algorithmic"] = row["oci_dense_factor_frac_of_fp64_peak_executed"] / 3.0
+            del sol
+        out.append(row)
+    return {"empty_launch_us": floor, "rows": out}
+
+
+def run_true_error(p, device):
+    """what the stop rule leaves. Per dt of the sweep, first time step from the initial condition:
+    |phi(tol 1e-8, rule 0) - phi(tol 1e-13)|_inf, for OCI and SI, and the same with the paper's rule (Eq. 12-13)."""
+    from paper_2503_00264_b200 import OCISolver
+    rows = []
+    for dt in SWEEP:
+        tight = OCISolver(p, dt=dt, device=device)
+        it_t, _, _ = tight.step(tol=1e-13, max_iters=20000, check_every=CHECK_EVERY, advance=False)
+        ref = tight.scalar_flux()
+        row = {"dt": dt, "tight_iters": it_t}
+        for key, fn, rule in (("oci_rule0", "step", 0), ("oci_rule1_paper", "step", 1), ("si_rule0", "si_step", 0)):
+            s_ = OCISolver(p, dt=dt, device=device)
+            it, _, _ = getattr(s_, fn)(tol=TOL, max_iters=20000, check_every=CHECK_EVERY, stop_rule=rule, advance=False)
+            row[key] = {"iters": it, "true_error_inf": float((s_.scalar_flux() - ref).abs().max().item())}
+            del s_
+        rows.append(row)
+        del tight
+    return rows
+
+
+def run_as_specified(p, device, no_si):
+    """BASELINE.json config 5 as written: for every dt of the sweep 10 time steps; a1 + a2 once per dt (the matrices do
+    not change inside a block)."""
+    import torch
+    from paper_2503_00264_b200 import OCISolver
+    oci, si = OCISolver(p, dt=SWEEP[0], device=device), OCISolver(p, dt=SWEEP[0], device=device)
+    rows, tot_ms, tot_it = [], 0.0, 0
+    for dt in SWEEP:
+        row = {"dt": dt, "steps": p.n_steps}
+        oci.set_dt(dt)
+        torch.cuda.synchronize(); t = time.perf_counter()
+        its = [oci.step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)[0] for _ in range(p.n_steps)]
+        row["oci_ms_total"] = (time.perf_counter() - t) * 1e3
+        row["oci_iters"] = its
+        row["oci_ms_per_step"] = row["oci_ms_total"] / p.n_steps
+        tot_ms += row["oci_ms_total"]; tot_it += sum(its)
+        if not no_si:
+            si.set_dt(dt)
+            torch.cuda.synchronize(); t = time.perf_counter()
+            its = [si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)[0] for _ in range(p.n_steps)]
+            row["si_ms_per_step"] = (time.perf_counter() - t) * 1e3 / p.n_steps
+            row["si_iters"] = its
+        rows.append(row)
+    return {"what": "config 5 as specified: 10 steps per dt, factors computed once per dt", "rows": rows,
+            "oci_cell_solves_per_s": p.J * tot_it / (tot_ms * 1e-3), "oci_ms_total": tot_ms, "oci_iterations_total": tot_it}
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -461,6 +620,8 @@ def main():
     ap.add_argument("--ref-cells", type=int, default=8192, help="cells per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-si", action="store_true", help="skip the SI comparator leg (profiling runs)")
+    ap.add_argument("--quick", action="store_true",
+                    help="skip the per_config / true_error / as_specified legs (profiling runs)")
     ap.add_argument("--table2", action="store_true",
                     help="instead of the headline benchmark: the paper's Table-2 delta sweep, OCI vs SI (SURVEY 8f row f3)")
     args = ap.parse_args()

@@ -175,6 +175,10 @@ int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host);/* what
                                                                           (OCI_E_UNSUPPORTED in solve_mode 1) */
 int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev);               /* [J][n] c_j of a3 [async]       */
 
+/* Enqueues `count` launches of an empty kernel (one CTA per SM) on the context's stream: the launch floor that the
+ * per-iteration times of the L2-resident configurations (BASELINE.json configs 1-2) are quoted against. [async] */
+int oci_debug_empty_launches(oci_ctx *ctx, int32_t count);
+
 /* Device time (ms, CUDA events on the context's stream) of the most recent call of each kind:
  * which 0 = oci_factor, 1 = oci_iterate / the iterations inside oci_step, 2 = si_iterate / si_step iterations.
  * *launches = kernels launched by that call. [sync] */

@@ -61,6 +61,7 @@ _SIGNATURES = {
     "oci_debug_get_inverse": (C.c_int, [_dptr, _i32, _dptr]),
     "oci_debug_get_factor_input": (C.c_int, [_dptr, _i32, _dptr]),
     "oci_debug_get_const_rhs": (C.c_int, [_dptr, _dptr]),
+    "oci_debug_empty_launches": (C.c_int, [_dptr, _i32]),
     "oci_last_timing": (C.c_int, [_dptr, _i32, C.POINTER(_f64), C.POINTER(_i64)]),
 }
 
@@ -284,6 +285,9 @@ class OCISolver:
         out = self._new(self.J, self.n)
         self._check("oci_debug_get_const_rhs", self.lib.oci_debug_get_const_rhs(self._ctx, out.data_ptr()))
         return out
+
+    def debug_empty_launches(self, count: int):
+        self._check("oci_debug_empty_launches", self.lib.oci_debug_empty_launches(self._ctx, int(count)))
 
     def last_timing(self, which: int):
         """(ms, launches) of the most recent factor (0) / OCI iterations (1) / SI iterations (2)."""

@@ -688,6 +688,18 @@ int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev)
     return 0;
 }
 
+int oci_debug_empty_launches(oci_ctx *ctx, int32_t count)
+{
+    if (!ctx) return -1;
+    DeviceGuard guard(ctx->device);
+    if (count < 0) return -2;
+    for (int i = 0; i < count; ++i) {
+        int r = launch_empty(ctx);
+        if (r < 0) return r;
+    }
+    return 0;
+}
+
 int oci_last_timing(oci_ctx *ctx, int32_t which, double *ms, int64_t *launches)
 {
     if (!ctx) return -1;

@@ -173,6 +173,7 @@ int launch_factor(oci_ctx *ctx);
 int launch_assemble_one(oci_ctx *ctx, int cell, double *A_dev_rowmajor);
 int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor);
 int launch_const_rhs(oci_ctx *ctx);
+int launch_empty(oci_ctx *ctx);
 int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 StopCheck make_stop(const oci_ctx *ctx, int slot, bool check_prev);
 int launch_advance(oci_ctx *ctx);

@@ -514,6 +514,12 @@ __global__ void scalar_flux_kernel(int J, int N, int G, const double *__restrict
     }
 }
 
+// the launch floor bench.py quotes the per-iteration times of the L2-resident configurations against
+__global__ void empty_kernel(int *sink)
+{
+    if (sink == nullptr && threadIdx.x == 1024) *sink = 0; // never true: keeps the kernel from being optimised away
+}
+
 inline int grid_for(size_t total, int threads, int num_sms)
 {
     size_t g = (total + threads - 1) / threads;
@@ -632,6 +638,13 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
     OCI_CUDA_TRY(ctx, cudaGetLastError());
     if (ctx->opt_ordering == 1) return 2; // red-black updates the current iterate in place: no buffer swap
     ctx->cur ^= 1;
+    return 1;
+}
+
+int launch_empty(oci_ctx *ctx)
+{
+    empty_kernel<<<ctx->num_sms, 160, 0, ctx->stream>>>(ctx->ctrl);
+    OCI_CUDA_TRY(ctx, cudaGetLastError());
     return 1;
 }
 
