@@ -487,11 +487,11 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 // (leading dimension ld). Same operations in the same order as a_entry(): bit-identical (asserted by
 // tests/test_gpu_parity.py::test_production_assembly_bit_exact through oci_debug_get_factor_input).
 __device__ __forceinline__ void assemble_rows2(const ProblemView &P, int cell, int lane, double *W, int ld,
-                                               int bmc0 = 0, int bmc_step = 1)
+                                               int bmc0 = 0, int bmc_step = 1, int rb0 = 0, int rb_step = 64)
 {
     const int N = P.N, G = P.G, NB = N * G;
     const double dx = P.dx[cell];
-    for (int rb = 0; rb < P.n; rb += 64) { // row block: rows rb + 2 lane, + 1
+    for (int rb = rb0; rb < P.n; rb += rb_step) { // row block: rows rb + 2 lane, + 1
         const int p0 = (lane & 1) * 2;
         const int bm = (rb >> 2) + (lane >> 1), m = bm % N, g = bm / N;
         const double sig = P.sigma_t[(size_t)cell * G + g], mu = P.mu[m];
@@ -1006,6 +1006,257 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
     }
 }
 
+// ============================================================================================================
+// n = 128: one CTA (one SM) per cell -- the production a1 + a2 kernel of config 3 and of the paper's S16 Table-2 problem.
+// ============================================================================================================
+// The design of factor_wc2_kernel at the size where one working matrix (132 KB) fills an SM: column-major W in shared
+// memory (leading dimension 132 = 4 mod 16, columns of a block in the order 0 2 1 3 4 6 5 7: conflict-free), panels
+// of 8 columns, rank-8 updates as transposed m8n8k4 DMMAs with the pivot rows zeroed instead of Z = T - I formed,
+// look-ahead, optimistic branch-free panel with an exact replay on a tie of high key words. What differs:
+//   * FOUR pivot warps, one row per lane (a single warp with four rows per lane would issue ~200 instructions per
+//     pivot step in order). Per step each warp finds its own first maximal |entry| (redux + ballot), its winner
+//     publishes {64-bit key, lane, row as it stands, 1 / candidate} in a slot, one named barrier over the 128 pivot
+//     threads, every lane picks the maximal key (strict >: a tie goes to the lower warp = the lower row) and
+//     eliminates its row. Two slot sets alternate, so one barrier per step.
+//   * Look-ahead: the pivot warps update the next panel's block -- warp w the row tiles 4 w .. 4 w + 3, which are the
+//     rows it then loads for the next panel, so nothing but one pivot-warp barrier (pivot rows read before anybody
+//     stores) separates update and panel -- while the four update warps apply the update to the other 14 blocks.
+constexpr int P128_LD = 132, P128_THREADS = 256, P128_AW = 4;
+
+struct alignas(16) P128Slot {
+    double row[FR_NB];
+    unsigned long long key; // |candidate| as an integer key (0: this warp has no unused row)
+    int lane;               // lane of the candidate; bit 8: more lanes of the warp share its high key word
+    int pad;
+    double linv, pad2;
+};
+
+struct P128Shared {
+    double W[128 * P128_LD];          // [column][row]
+    P128Slot slot[2][P128_AW];        // [step parity][pivot warp]
+    int rho[128], rhoinv[128];
+    int cell, sing, tie;
+};
+
+__device__ __forceinline__ void p128_bar_pivot() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+template <int b, bool FAST>
+__device__ __forceinline__ void p128_pivot_step(double (&t)[FR_NB], unsigned &m, P128Shared &sh, int w, int lane, int col0,
+                                                unsigned &bad, unsigned &tie)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    const unsigned h = (unsigned)__double2hiint(t[b]) & m, l = (unsigned)__double2loint(t[b]);
+    const unsigned mh = __reduce_max_sync(FULL, h);
+    const double linv = rcp_nr(t[b]); // in the shadow of the reduction
+    unsigned ball = __ballot_sync(FULL, h == mh);
+    const unsigned tied = ball & (ball - 1u); // more than one lane of this warp holds its maximal high word
+    if (!FAST && tied) { // low words, then the lowest lane (= the lowest row)
+        const bool cand = h == mh;
+        const unsigned ml = __reduce_max_sync(FULL, cand ? l : 0u);
+        ball = __ballot_sync(FULL, cand && l == ml);
+    }
+    const int src = (__ffs(ball) - 1) & 31;
+    P128Slot *mine = &sh.slot[b & 1][w];
+    if (lane == src) { // this warp's candidate: key, row as it stands, 1 / candidate
+#pragma unroll
+        for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(mine->row)[c] = make_double2(t[2 * c], t[2 * c + 1]);
+        mine->linv = linv;
+        mine->key = ((unsigned long long)h << 32) | l; // h == 0: no unused row here (loses, or the cell is singular)
+        mine->lane = lane | (tied ? 0x100 : 0);
+    }
+    p128_bar_pivot();
+    // the four candidates: key and lane word of a slot in one 16-byte broadcast load
+    unsigned long long kk[P128_AW];
+    int lw4[P128_AW];
+#pragma unroll
+    for (int ww = 0; ww < P128_AW; ++ww) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(&sh.slot[b & 1][ww].key);
+        kk[ww] = ((unsigned long long)v.y << 32) | v.x;
+        lw4[ww] = (int)v.z;
+    }
+    unsigned long long kmax = kk[0];
+    int gw = 0, lwv = lw4[0];
+#pragma unroll
+    for (int ww = 1; ww < P128_AW; ++ww) // strict >: a tie goes to the lower warp, i.e. the lower row
+        if (kk[ww] > kmax) { kmax = kk[ww]; gw = ww; lwv = lw4[ww]; }
+    if (FAST) { // an unresolved tie matters only where it could have hidden the true maximum: in a warp whose published
+                // high word equals the winning one (most warps tie on the identical entries -dx K w / 4 of Eq. 10, far
+                // below the pivot)
+#pragma unroll
+        for (int ww = 0; ww < P128_AW; ++ww)
+            if ((lw4[ww] & 0x100) && (unsigned)(kk[ww] >> 32) == (unsigned)(kmax >> 32)) tie |= 1u;
+    }
+    bad |= ((unsigned)(kmax >> 32) - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot
+    const P128Slot *win = &sh.slot[b & 1][gw];
+    const double ls = win->linv;
+    const int lw = lwv & 31;
+    double sp[FR_NB];
+#pragma unroll
+    for (int c = 0; c < FR_NB; ++c) sp[c] = (c == b) ? ls : win->row[c] * ls;
+    const bool is_p = gw == w && lane == lw;
+    const double f = t[b];
+#pragma unroll
+    for (int c = 0; c < FR_NB; ++c) {
+        const double u = (c == b) ? -f * ls : fma(-f, sp[c], t[c]);
+        t[c] = is_p ? sp[c] : u;
+    }
+    m = is_p ? 0u : m;
+    if (w == 0 && lane == b) {
+        const int r = 32 * gw + lw;
+        sh.rho[col0 + b] = r;
+        sh.rhoinv[r] = col0 + b;
+    }
+}
+
+template <bool FAST>
+__device__ __forceinline__ void p128_panel(double (&t)[FR_NB], unsigned &m, P128Shared &sh, int w, int lane, int col0,
+                                           unsigned &bad, unsigned &tie)
+{
+    p128_pivot_step<0, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<1, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<2, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<3, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<4, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<5, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<6, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    p128_pivot_step<7, FAST>(t, m, sh, w, lane, col0, bad, tie);
+}
+
+// one whole column block by one warp (see wc2_update_blocks): pivot rows read, zeroed, 16 row tiles updated
+__device__ __forceinline__ void p128_update_block(double *W, int Jb, const double (&zf)[16][2], int rk0, int rk1, int lq, int lg)
+{
+    constexpr int LD = P128_LD;
+    const int cl = wc2_colmap(lg);
+    double *a0p = &W[(8 * Jb + cl) * LD + rk0], *a1p = &W[(8 * Jb + cl) * LD + rk1];
+    const double a0 = *a0p, a1 = *a1p;
+    __syncwarp();
+    *a0p = 0.0;
+    *a1p = 0.0;
+    __syncwarp();
+    double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]);
+#pragma unroll
+    for (int I = 0; I < 16; ++I) {
+        double2 v = cp[4 * I];
+        dmma884(v.x, v.y, a0, zf[I][0]);
+        dmma884(v.x, v.y, a1, zf[I][1]);
+        cp[4 * I] = v;
+    }
+}
+
+template <bool DUMP>
+__global__ void __launch_bounds__(P128_THREADS, 1)
+factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_cell, double *__restrict__ dumpA, int dump_cell)
+{
+    constexpr int n = 128, LD = P128_LD, NPANEL = n / FR_NB;
+    extern __shared__ __align__(16) unsigned char p128_smem[];
+    P128Shared &sh = *reinterpret_cast<P128Shared *>(p128_smem);
+    double *W = sh.W;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
+    const bool roleA = w < P128_AW;
+
+    for (;;) {
+        if (threadIdx.x == 0) { sh.cell = DUMP ? dump_cell : atomicAdd(next_cell, 1); sh.sing = 0; sh.tie = 0; }
+        __syncthreads();
+        const int cell = sh.cell;
+        if (cell >= P.J) break;
+        assemble_rows2(P, cell, lane, W, LD, w >> 1, 4, 64 * (w & 1), 128);
+        __syncthreads();
+        if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
+            for (int e = threadIdx.x; e < n * n; e += P128_THREADS) dumpA[e] = W[(e & 127) * LD + (e >> 7)];
+            break;
+        }
+
+        double t[FR_NB];            // pivot warps: row 32 w + lane of the current panel
+        unsigned m = 0x7fffffffu;   // 0 once that row has been a pivot row
+        bool singular = false;
+        for (int pnl = 0; pnl < NPANEL; ++pnl) {
+            if (roleA) {
+                const int r = 32 * w + lane;
+                double *Wp = &W[(FR_NB * pnl) * LD + r];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
+                unsigned bad = 0u, tie = 0u;
+                const unsigned m_in = m;
+                p128_panel<true>(t, m, sh, w, lane, FR_NB * pnl, bad, tie);
+                if (tie) sh.tie = 1;
+                p128_bar_pivot();
+                const bool redo = sh.tie != 0;
+                p128_bar_pivot();
+                if (redo) { // pivot-warp-uniform and rare: the panel again, from shared memory, ties resolved exactly
+                    if (threadIdx.x == 0) sh.tie = 0;
+#pragma unroll
+                    for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
+                    m = m_in;
+                    bad = 0u;
+                    p128_panel<false>(t, m, sh, w, lane, FR_NB * pnl, bad, tie);
+                }
+                if (bad && threadIdx.x == 0) sh.sing = 1;
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) Wp[c * LD] = t[c]; // the eliminated panel (T e_r) back in place
+            }
+            __syncthreads(); // barrier p: T(p), R(p) visible to everybody; update p - 1 is complete
+            if (sh.sing) { singular = true; break; } // CTA-uniform
+
+            // ================= phase U: rank-8 update of the other 120 columns =================
+            const int rk0 = sh.rho[FR_NB * pnl + lq], rk1 = sh.rho[FR_NB * pnl + 4 + lq];
+            double zf[16][2]; // B fragments: T[8 I + lg][panel column 4 h + lq]
+#pragma unroll
+            for (int I = 0; I < 16; ++I) {
+                zf[I][0] = W[(FR_NB * pnl + lq) * LD + 8 * I + lg];
+                zf[I][1] = W[(FR_NB * pnl + 4 + lq) * LD + 8 * I + lg];
+            }
+            if (pnl + 1 < NPANEL) {
+                if (roleA) {
+                    // look-ahead: the next panel's block, pivot warp w its own 32 rows (row tiles 4 w .. 4 w + 3). Z = T - I
+                    // explicitly here (zeroing the pivot rows would cost a second pivot-warp barrier).
+                    const int Jb = pnl + 1, cl = wc2_colmap(lg);
+                    const double a0 = W[(8 * Jb + cl) * LD + rk0], a1 = W[(8 * Jb + cl) * LD + rk1];
+                    p128_bar_pivot(); // every pivot warp has read the pivot rows of the block
+                    double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]);
+#pragma unroll
+                    for (int I = 0; I < 16; ++I) {
+                        if ((I >> 2) != w) continue;
+                        const int row = 8 * I + lg;
+                        double2 v = cp[4 * I];
+                        dmma884(v.x, v.y, a0, zf[I][0] - (rk0 == row ? 1.0 : 0.0));
+                        dmma884(v.x, v.y, a1, zf[I][1] - (rk1 == row ? 1.0 : 0.0));
+                        cp[4 * I] = v;
+                    }
+                    __syncwarp();
+                } else {
+                    for (int Jb = w - P128_AW; Jb < NPANEL; Jb += P128_THREADS / 32 - P128_AW)
+                        if (Jb != pnl && Jb != pnl + 1) p128_update_block(W, Jb, zf, rk0, rk1, lq, lg);
+                }
+            } else { // last panel: the other 15 blocks shared out over all eight warps
+                for (int Jb = w; Jb < NPANEL - 1; Jb += P128_THREADS / 32) p128_update_block(W, Jb, zf, rk0, rk1, lq, lg);
+            }
+        }
+        __syncthreads(); // the last update is complete
+
+        double *out = Minv + (size_t)cell * n * n;
+        if (singular) {
+            if (threadIdx.x == 0) atomicMin(info, cell + 1);
+            for (int e = threadIdx.x; e < n * n / 2; e += P128_THREADS) reinterpret_cast<double2 *>(out)[e] = make_double2(0.0, 0.0);
+            __syncthreads();
+            continue;
+        }
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j] (rows scattered on the way out, see wc2)
+        int ro[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) ro[q] = sh.rhoinv[64 * (q >> 1) + 2 * lane + (q & 1)];
+        for (int j = w; j < n; j += P128_THREADS / 32) {
+            const double2 v0 = *reinterpret_cast<const double2 *>(&W[j * LD + 2 * lane]);
+            const double2 v1 = *reinterpret_cast<const double2 *>(&W[j * LD + 64 + 2 * lane]);
+            double *col = out + (size_t)sh.rho[j] * n;
+            col[ro[0]] = v0.x;
+            col[ro[1]] = v0.y;
+            col[ro[2]] = v1.x;
+            col[ro[3]] = v1.y;
+        }
+        __syncthreads(); // everybody is done with W and sh.cell before the next cell
+    }
+}
+
 __global__ void assemble_one_kernel(ProblemView P, int cell, double *__restrict__ A)
 {
     const int n = P.n;
@@ -1118,12 +1369,34 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
     return 1;
 }
 
+// n = 128, one CTA per cell (factor_p128_kernel). dumpA != nullptr: only assemble `dump_cell` and write the tile there.
+static int launch_factor_p128(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
+{
+    const size_t smem = sizeof(P128Shared);
+    const void *fn = dumpA ? (const void *)factor_p128_kernel<true> : (const void *)factor_p128_kernel<false>;
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int grid = 1;
+    if (!dumpA) {
+        grid = ctx->num_sms;
+        if (grid > ctx->J) grid = ctx->J;
+        OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info + 1, 0, sizeof(int), ctx->stream)); // the cell counter
+    }
+    int *counter = ctx->info + 1;
+    double *Minv = ctx->Minv;
+    int *info = ctx->info;
+    ProblemView Pv = P;
+    void *args[] = {&Pv, &Minv, &info, &counter, &dumpA, &dump_cell};
+    OCI_CUDA_TRY(ctx, cudaLaunchKernel(fn, dim3(grid), dim3(P128_THREADS), args, smem, ctx->stream));
+    return 1;
+}
+
 int launch_factor(oci_ctx *ctx)
 {
     const int n = ctx->n;
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream)); // 0x7f7f7f7f = "none"
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && n == 64) return launch_factor_wc(ctx, P, nullptr, 0);
+    if (ctx->opt_factor_kernel == 1 && n == 128) return launch_factor_p128(ctx, P, nullptr, 0);
     if (ctx->opt_factor_kernel >= 1 && n % 64 == 0 && n <= 256) // 2: the 8-warp kernel also for n = 64
         return launch_factor_reg_n(ctx, P, nullptr, 0);
     const bool global_w = factor_smem_bytes(n, false) > (size_t)ctx->max_smem_optin;
@@ -1156,6 +1429,7 @@ int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor)
     ProblemView P = make_view(ctx);
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && ctx->n == 64)
         return launch_factor_wc(ctx, P, A_dev_rowmajor, cell);
+    if (ctx->opt_factor_kernel == 1 && ctx->n == 128) return launch_factor_p128(ctx, P, A_dev_rowmajor, cell);
     if (ctx->opt_factor_kernel >= 1 && ctx->n % 64 == 0 && ctx->n <= 256) return launch_factor_reg_n(ctx, P, A_dev_rowmajor, cell);
     return 0;
 }
