@@ -151,8 +151,10 @@ int one_iteration(oci_ctx *ctx, int scheme, int slot, bool want_l2, bool check_p
 // the one before it and skips itself once the stop rule held (device-side stop). Returns kernels launched.
 int issue_batch(oci_ctx *ctx, int scheme, int slot0, int k, bool want_l2, bool check_between)
 {
-    if (scheme == 0) {
-        const int r = launch_st_multi(ctx, slot0, k, want_l2, check_between); // one cooperative launch, if it applies
+    if (scheme == 0) { // one cooperative launch for the whole batch, where that applies
+        int r = launch_st_multi(ctx, slot0, k, want_l2, check_between);
+        if (r != 0) return r;
+        r = launch_dense_multi(ctx, slot0, k, want_l2, check_between);
         if (r != 0) return r;
     }
     int launches = 0;

@@ -21,7 +21,8 @@ enum { // one slot per kernel instantiation that needs more than 48 KB of dynami
     SLOT_STREAM = 6,   // + want_l2                     (2 slots)
     SLOT_SWEEP = 8,    // + lanes index                 (3 slots)
     SLOT_STP = 11,     // + ((GC index) * 2 + CT index) * 2 + want_l2   (20 slots)
-    SLOT_FACTOR = 32   // factor kernels
+    SLOT_FACTOR = 32,  // factor kernels
+    SLOT_RESIDENT = 40 // + want_l2 (2 slots)
 };
 
 // ------------------------------------------------------------------------------------------------------------
@@ -185,6 +186,7 @@ int launch_st_factor(oci_ctx *ctx);
 int launch_st_iteration(oci_ctx *ctx, const struct IterParams &P, bool want_l2);
 // `k` structured iterations (history slots slot0 .. slot0 + k - 1) in ONE cooperative launch; 0 = not applicable
 int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_between);
+int launch_dense_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_between);
 int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 
 #ifdef __CUDACC__

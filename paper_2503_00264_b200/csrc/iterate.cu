@@ -14,6 +14,7 @@
 // the chunks as they land: oci_iterate_wpc_kernel (n = 64, 128, 256: a cell per consumer warp, the production
 // kernel of configs 3-5) and oci_iterate_stream_kernel (any other n: a team of threads per cell).
 #include "common.cuh"
+#include <cooperative_groups.h>
 
 namespace {
 
@@ -467,6 +468,110 @@ __global__ void __launch_bounds__(256) oci_iterate_plain_kernel(const IterParams
     }
 }
 
+// ============================================================================================================
+// SURVEY 8(f) row f2, dense path: resident multi-iteration kernel for problems whose inverses fit in the shared memory
+// of the chip (BASELINE.json configs 1-2: 32 KB and 8.4 MB of A_j^{-1}).
+// ============================================================================================================
+// PAPER.md:413-415 notes that on small problems the iteration loop is bound by dispatch, not by work. Here ONE
+// cooperative launch runs up to n_iters block-Jacobi iterations: every CTA copies the inverses and the constant
+// right-hand sides of its contiguous range of cells into shared memory ONCE and keeps them there, an iteration reads
+// only Psi^(l) of its cells and their two neighbours (written by other CTAs of the same launch: past the L1), and a
+// grid-wide barrier separates the iterations. Same arithmetic per cell as the other dense kernels, same device-side
+// stop: after the barrier every thread of the grid reads the same residual slot and takes the same decision.
+struct DenseMulti {
+    int n_iters, slot0, check_between, rule, cpc; // cpc: cells per CTA
+    double tol;
+    unsigned long long *resid_inf; // history base (slot 0)
+    double *resid_l2;
+    int *executed;
+};
+
+template <bool WANT_L2>
+__global__ void __launch_bounds__(256) oci_iterate_resident_kernel(const IterParams P, const DenseMulti M)
+{
+    extern __shared__ __align__(16) unsigned char rs_smem[];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const int n = P.n, N = P.N, G = P.G, J = P.J, cpc = M.cpc;
+    const int cell0 = blockIdx.x * cpc, nc = max(0, min(cpc, J - cell0));
+    double *Ms = reinterpret_cast<double *>(rs_smem);   // [cpc][n(col)][n(row)]
+    double *cs = Ms + (size_t)cpc * n * n;               // [cpc][n]   c_j
+    double *bs = cs + (size_t)cpc * n;                   // [cpc][n]   b_j, then Psi^(l+1)
+    double *nb = bs + (size_t)cpc * n;                   // [cpc + 2][n] Psi^(l) of cells cell0 - 1 .. cell0 + cpc
+    double *mu_s = nb + (size_t)(cpc + 2) * n;           // [N]
+    double *w_s = mu_s + N;                              // [N]
+    double *red = w_s + N;                               // [8] block reduction scratch
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < N; i += blockDim.x) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    for (size_t e = tid; e < (size_t)nc * n * n; e += blockDim.x) Ms[e] = P.Minv[(size_t)cell0 * n * n + e];
+    for (int e = tid; e < nc * n; e += blockDim.x) cs[e] = P.c[(size_t)cell0 * n + e];
+    const double *psi_old = P.psi_old;
+    double *psi_new = P.psi_new;
+    for (int it = 0; it < M.n_iters; ++it) {
+        const int slot = M.slot0 + it;
+        if (M.check_between && it > 0) {
+            StopCheck st;
+            st.prev_inf = M.resid_inf + slot - 1;
+            st.prev_l2 = M.resid_l2 + slot - 1;
+            st.prev2_l2 = slot >= 2 ? M.resid_l2 + slot - 2 : nullptr;
+            st.tol = M.tol; st.rule = M.rule; st.slot = slot; st.executed = M.executed;
+            if (stop_reached_t<true>(st)) break; // same values everywhere: the whole grid leaves together
+        }
+        if (blockIdx.x == 0 && tid == 0) *M.executed = slot + 1;
+        // Psi^(l) of the own cells and the two neighbours (zeros outside the slab; boundary cells use the BC instead)
+        for (int e = tid; e < (nc + 2) * n; e += blockDim.x) {
+            const int jj = cell0 - 1 + e / n;
+            nb[e] = (jj >= 0 && jj < J) ? __ldcg(psi_old + (size_t)jj * n + (e % n)) : 0.0;
+        }
+        __syncthreads();
+        for (int e = tid; e < nc * n; e += blockDim.x) // a4: b = c + incident(Psi^(l))
+            bs[e] = cs[e] + incident_term(P, nb, cell0, cell0 + e / n, e % n, mu_s);
+        __syncthreads();
+        double rmax = 0.0, l2 = 0.0, x_first = 0.0;
+        for (int e = tid; e < nc * n; e += blockDim.x) { // a5: x = A^{-1} b (one entry per thread at the intended sizes)
+            const int a = e / n, i = e - a * n;
+            const double *Mp = Ms + (size_t)a * n * n + i, *bp = bs + a * n;
+            double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+            int c = 0;
+            for (; c + 3 < n; c += 4) {
+                acc0 = fma(Mp[(size_t)c * n], bp[c], acc0);
+                acc1 = fma(Mp[(size_t)(c + 1) * n], bp[c + 1], acc1);
+                acc2 = fma(Mp[(size_t)(c + 2) * n], bp[c + 2], acc2);
+                acc3 = fma(Mp[(size_t)(c + 3) * n], bp[c + 3], acc3);
+            }
+            for (; c < n; ++c) acc0 = fma(Mp[(size_t)c * n], bp[c], acc0);
+            const double x = (acc0 + acc1) + (acc2 + acc3);
+            if (e == tid) x_first = x;
+            psi_new[(size_t)cell0 * n + e] = x;
+            if (WANT_L2) { const double d = x - nb[n + e]; l2 = fma(d, d, l2); }
+        }
+        __syncthreads(); // everybody has read bs: it now receives Psi^(l+1) for the phi reduction
+        for (int e = tid; e < nc * n; e += blockDim.x) bs[e] = e == tid ? x_first : psi_new[(size_t)cell0 * n + e];
+        __syncthreads();
+        for (int e = tid; e < nc * G * 4; e += blockDim.x) { // a6 + a7
+            const int p = e & 3, ag = e >> 2, g = ag % G, a = ag / G;
+            const double *xn = bs + a * n + g * N * 4 + p, *xo = nb + (a + 1) * n + g * N * 4 + p;
+            double sn = 0.0, so = 0.0;
+            for (int m = 0; m < N; ++m) { sn = fma(w_s[m], xn[m * 4], sn); so = fma(w_s[m], xo[m * 4], so); }
+            P.phi[(size_t)cell0 * G * 4 + e] = sn;
+            const double d = fabs(sn - so);
+            rmax = (d > rmax || !(d == d)) ? d : rmax;
+        }
+        rmax = warp_max(rmax);
+        if (lane == 0) red[warp] = rmax;
+        if (WANT_L2) { l2 = warp_sum(l2); if (lane == 0 && nc > 0) atomicAdd(M.resid_l2 + slot, l2); }
+        __syncthreads();
+        if (tid == 0 && nc > 0) {
+            double r = red[0];
+            for (int q = 1; q < (int)(blockDim.x >> 5); ++q) r = (red[q] > r || !(red[q] == red[q])) ? red[q] : r;
+            atomicMax(M.resid_inf + slot, resid_bits(r));
+        }
+        grid.sync();
+        const double *t = psi_old;
+        psi_old = psi_new;
+        psi_new = const_cast<double *>(t);
+    }
+}
+
 // ---- a3: constant part of b_j (Eq. 9c-d without the incident terms; 4th row of 9c restored,
 // DESIGN.md A1): rows (k,L),(k,R): dx/4 Q_k + dx/(2 v dt) psi_{k-1/2}; rows (k+1/2,L),(k+1/2,R): dx/4 Q_{k+1/2}
 __global__ void const_rhs_kernel(ProblemView P, const double *__restrict__ q, const double *__restrict__ psi_prev,
@@ -680,5 +785,46 @@ int launch_scalar_flux(oci_ctx *ctx, const double *psi, double *phi)
     const size_t total = (size_t)ctx->J * ctx->G * 4;
     scalar_flux_kernel<<<grid_for(total, 256, ctx->num_sms), 256, 0, ctx->stream>>>(ctx->J, ctx->N, ctx->G, ctx->w, psi, phi);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
+    return 1;
+}
+
+// f2, dense path: k iterations in one cooperative launch with the inverses resident in shared memory. Applies (auto)
+// when the problem's inverses fit in the shared memory of the chip with one CTA per SM; "persistent" = 0 disables it.
+// Returns 0 when it does not apply (the caller falls back to one launch per iteration).
+int launch_dense_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_between)
+{
+    if (ctx->opt_solve_mode != 0 || ctx->opt_persistent == 0 || ctx->opt_ordering != 0 || k < 2) return 0;
+    if (ctx->opt_iterate_kernel == 0) return 0; // the plain kernel was asked for
+    const int n = ctx->n;
+    int grid = ctx->num_sms < ctx->J ? ctx->num_sms : ctx->J;
+    const int cpc = (ctx->J + grid - 1) / grid;
+    grid = (ctx->J + cpc - 1) / cpc;
+    const size_t smem = sizeof(double) * ((size_t)cpc * n * n + (size_t)(3 * cpc + 2) * n + 2 * (size_t)ctx->N + 8);
+    if (smem > (size_t)ctx->max_smem_optin) return 0;
+    int coop = 0;
+    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess || !coop) return 0;
+    const void *fn = want_l2 ? (const void *)oci_iterate_resident_kernel<true> : (const void *)oci_iterate_resident_kernel<false>;
+    OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_RESIDENT + (want_l2 ? 1 : 0), fn, smem));
+    int per_sm = 0;
+    OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, smem));
+    if (per_sm < 1 || grid > per_sm * ctx->num_sms) return 0; // all CTAs must be co-resident for the grid barrier
+    IterParams P;
+    P.stop = make_stop(ctx, slot0, false);
+    P.J = ctx->J; P.N = ctx->N; P.G = ctx->G; P.n = n;
+    P.bc_left = ctx->bc_left; P.bc_right = ctx->bc_right;
+    P.Minv = ctx->Minv; P.c = ctx->c;
+    P.psi_old = ctx->psi[ctx->cur]; P.psi_new = ctx->psi[ctx->cur ^ 1];
+    P.phi = ctx->phi; P.mu = ctx->mu; P.w = ctx->w;
+    P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
+    P.resid_inf = ctx->resid_inf + slot0; P.resid_l2 = ctx->resid_l2 + slot0;
+    P.cpb = 1; P.S = 1; P.cw = n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
+    P.color = 0; P.ncolors = 1;
+    DenseMulti M;
+    M.n_iters = k; M.slot0 = slot0; M.check_between = check_between ? 1 : 0; M.rule = ctx->stop_rule; M.tol = ctx->stop_tol;
+    M.cpc = cpc;
+    M.resid_inf = ctx->resid_inf; M.resid_l2 = ctx->resid_l2; M.executed = ctx->ctrl;
+    void *args[] = {&P, &M};
+    OCI_CUDA_TRY(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, ctx->stream));
+    if (k & 1) ctx->cur ^= 1; // as k single launches would have left it
     return 1;
 }

@@ -502,3 +502,51 @@ def test_redblack_needs_the_structured_path():
     s.factor()
     with pytest.raises(Exception):
         s.iterate(1)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# SURVEY 8(f) row f2, dense path: a batch of iterations as ONE cooperative launch with the inverses resident in shared
+# memory (automatic when they fit: BASELINE.json configs 1-2). Mirrors the test_persistent_* tests of the structured path.
+# ---------------------------------------------------------------------------------------------------------------
+def _fits_resident(J, N, G, sms=148, smem=200 * 1024):
+    """the inverses of ceil(J / SMs) cells fit in one CTA's shared memory (launch_dense_multi's condition, with margin)"""
+    n = 4 * N * G
+    return -(-J // sms) * n * n * 8 <= smem
+
+
+@pytest.mark.parametrize("seed,J,N,G,bl,br", [c for c in SMALL_CASES if _fits_resident(c[1], c[2], c[3])] + [(21, 1200, 8, 1, 1, 2)])
+def test_dense_resident_multi_iteration_parity(seed, J, N, G, bl, br):
+    p = W.random_problem(seed, J, N, G, bc_left=bl, bc_right=br)
+    s, o = _solver(p), _oracle(p)
+    assert s.factor() == 0 and o.factor() == 0
+    o.const_rhs()
+    for k in (2, 5, 8):          # even and odd batch lengths: the two Psi buffers alternate inside the launch
+        s.iterate(k)
+        assert s.last_timing(1)[1] <= 2, "the batch should have been ONE launch (+ the constant right-hand side the first time)"
+        o.oci_iterate(k)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_ITER, f"after a batch of {k}"
+        assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_ITER
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("k", [2, 5, 8])
+def test_dense_resident_step_loop_stops_at_the_natural_iteration(rule, k):
+    p = W.random_problem(33, 61, 4, 2, bc_left=1, bc_right=2, dt=0.05)
+    s, o = _solver(p), _oracle(p)
+    for step in range(3):
+        it_g, conv_g, _ = s.step(tol=1e-9, max_iters=500, check_every=k, stop_rule=rule)
+        it_o, hist_o = o.oci_step(tol=1e-9, max_iters=500, rule=rule)
+        assert it_g == conv_g == it_o, f"step {step}"
+        np.testing.assert_allclose(s.residual_history(kind=rule), hist_o, rtol=1e-6, atol=1e-15)
+        assert rel(s.angular_flux().cpu().numpy(), o.psi) < TOL_PHI
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+
+
+def test_dense_resident_auto_applies_to_config2_and_matches_the_per_iteration_kernel():
+    p = W.config2(dt=0.1)
+    a, b = _solver(p), _solver(p, options={"persistent": 0})
+    ia, _, _ = a.step(tol=p.tol, max_iters=4000, check_every=8)
+    ib, _, _ = b.step(tol=p.tol, max_iters=4000, check_every=8)
+    assert ia == ib
+    assert a.last_timing(1)[1] < b.last_timing(1)[1]          # one launch per batch instead of one per iteration
+    assert rel(a.scalar_flux().cpu().numpy(), b.scalar_flux().cpu().numpy()) < 1e-13
