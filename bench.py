@@ -609,6 +609,32 @@ def run_table2(args):
                       "stop_rule": "Eq. 12-13, eps = 1e-8", "rows": rows}))
 
 
+def run_factor_ab(args):
+    """The a1 + a2 kernels for n = 64 side by side on config 5 (the DMMA decision): the production
+    kernel (two warps per cell, look-ahead, DMMA), the one-warp-per-cell kernel with its rank-8 updates as DMMA and as
+    DFMA (everything else identical), and the register-tiled kernel of round 1. One JSON line."""
+    import torch
+    from paper_2503_00264_b200 import OCISolver
+    p = W.config5(dt=1e-3)
+    n, J = p.n, p.J
+    rows = []
+    for name, opts in (("factor_wc2_kernel: 2 warps/cell, look-ahead, DMMA [production]", {}),
+                       ("factor_wc_kernel<DMMA>: 1 warp/cell", {"factor_kernel": 4, "factor_update": 1}),
+                       ("factor_wc_kernel<DFMA>: 1 warp/cell", {"factor_kernel": 4, "factor_update": 0}),
+                       ("factor_reg_kernel<1>: register-tiled, DFMA (round 1)", {"factor_kernel": 2})):
+        s = OCISolver(p, options=opts)
+        ts = []
+        for r in range(4):
+            s.set_dt(p.dt * (1 + 1e-9 * (r + 1)))
+            assert s.factor() == 0
+            ts.append(s.last_timing(0)[0])
+        ms = min(ts[1:])
+        rows.append({"kernel": name, "ms": ms, "tflops_executed": 2.0 * n ** 3 * J / (ms * 1e-3) / 1e12,
+                     "frac_of_fp64_peak_executed": 2.0 * n ** 3 * J / (ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS})
+        del s
+    print(json.dumps({"experiment": "factor kernels for n = 64 on config 5 (J = 65536)", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -622,12 +648,16 @@ def main():
     ap.add_argument("--no-si", action="store_true", help="skip the SI comparator leg (profiling runs)")
     ap.add_argument("--quick", action="store_true",
                     help="skip the per_config / true_error / as_specified legs (profiling runs)")
+    ap.add_argument("--factor-ab", action="store_true",
+                    help="instead of the headline benchmark: the n = 64 factor kernels side by side (DMMA vs DFMA evidence)")
     ap.add_argument("--table2", action="store_true",
                     help="instead of the headline benchmark: the paper's Table-2 delta sweep, OCI vs SI (SURVEY 8f row f3)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.table2:
+    if args.factor_ab:
+        run_factor_ab(args)
+    elif args.table2:
         run_table2(args)
     elif args.impl == "reference":
         run_reference(args)
