@@ -78,7 +78,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering, opt_st_warp_local, opt_st_ct;
     // largest dynamic shared-memory size already granted (cudaFuncSetAttribute) to each kernel this context launches;
     // kept per context (= per device), never in function-local statics
     size_t smem_granted[OCI_SMEM_SLOTS];

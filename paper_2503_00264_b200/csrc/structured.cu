@@ -367,7 +367,8 @@ __host__ __device__ inline StStage st_stage_layout(int N, int G, int CT)
 
 // CT = consumer threads per CTA (256, or 128 so that four CTAs share an SM); one more warp holds the producer thread.
 template <bool WANT_L2, int GC, int CT>
-__global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_kernel(const IterParams P, const StParams S, int stages)
+__global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_kernel(const IterParams P, const StParams S, int stages,
+                                                                                     int warp_local)
 {
     if (stop_reached(P.stop)) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
@@ -384,7 +385,11 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
     double *phiz = wz + (size_t)CPB * GN * 4;                         // [CPB][4G]
     double *ys = phiz + (size_t)CPB * G4;                             // [CPB][4G]
     double *ss = ys + (size_t)CPB * G4;                               // [CPB][4G]
-    size_t off = (size_t)((unsigned char *)(ss + (size_t)CPB * G4) - stp_smem);
+    // prescribed incident fluxes in shared memory: a global load inside the batch body would share a scoreboard slot
+    // with the role-2 prefetch loads below and make every batch wait for them (ncu: 19 % of the samples, long_sb)
+    double *incl_s = ss + (size_t)CPB * G4;                           // [G N][2]
+    double *incr_s = incl_s + 2 * GN;                                 // [G N][2]
+    size_t off = (size_t)((unsigned char *)(incr_s + 2 * GN) - stp_smem);
     off = (off + 127) & ~(size_t)127;
     double *ring = reinterpret_cast<double *>(stp_smem + off);        // stages x lay.doubles
 
@@ -394,6 +399,10 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
         fence_mbar_init();
     }
     for (int i = tid; i < N; i += STP_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
+    for (int i = tid; i < 2 * GN; i += STP_THREADS) {
+        incl_s[i] = P.bc_left == OCI_BC_PRESCRIBED ? P.inc_left[i] : 0.0;
+        incr_s[i] = P.bc_right == OCI_BC_PRESCRIBED ? P.inc_right[i] : 0.0;
+    }
     __syncthreads();
 
     const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
@@ -436,9 +445,23 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
     };
     // butterfly reduction over the ordinates: N a power of two <= 32 (groups of N lanes never straddle a warp then)
     const bool shfl_reduce = N <= 32 && (N & (N - 1)) == 0;
+    // warp_local (host: GC > 0, N a power of two >= 4, G N <= 32): a cell's G N threads sit inside one warp and ALSO do
+    // the cell's 4G-row steps (thread (a, gm) takes row gm < 4G), so every exchange of a batch is warp-local and the
+    // batch needs no CTA barrier at all (ncu on the previous version: 28 % of the warp samples in bar.sync). For G = 1
+    // there is not even an exchange: the butterfly leaves phi_z in every lane, and each lane applies the 4 x 4 C^-1.
+    const bool wl = GC > 0 && warp_local != 0;
     double Kr_n[GC > 0 ? GC : 1], dxq_n = 0.0, phi_old_n = 0.0;
     auto load_role2 = [&](int gb_, int nb_) {
-        if (GC > 0 && tid < rows && tid / G4 < nb_) {
+        if (wl) {
+            if (a < nb_ && lane_on && (gm < G4 || GC == 1)) {
+                const int j2 = gb_ + a, r2 = gm < G4 ? gm : 0;
+                const double *Kp = S.transfer + ((size_t)j2 * G + (r2 >> 2)) * G;
+#pragma unroll
+                for (int gc = 0; gc < (GC > 0 ? GC : 1); ++gc) Kr_n[gc] = Kp[gc];
+                dxq_n = S.dx[j2];
+                if (gm < G4) phi_old_n = P.phi[(size_t)j2 * G4 + gm];
+            }
+        } else if (GC > 0 && tid < rows && tid / G4 < nb_) {
             const int a2 = tid / G4, r2 = tid - a2 * G4, j2 = gb_ + a2;
             const double *Kp = S.transfer + ((size_t)j2 * G + (r2 >> 2)) * G;
 #pragma unroll
@@ -479,7 +502,7 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
                 }
                 else if (P.bc_left == OCI_BC_REFLECTIVE) {
                     v0 = self[(g * N + (N - 1 - m)) * 4 + 0]; v1 = self[(g * N + (N - 1 - m)) * 4 + 2];
-                } else if (P.bc_left == OCI_BC_PRESCRIBED) { v0 = P.inc_left[gm * 2]; v1 = P.inc_left[gm * 2 + 1]; }
+                } else if (P.bc_left == OCI_BC_PRESCRIBED) { v0 = incl_s[gm * 2]; v1 = incl_s[gm * 2 + 1]; }
                 b[0] = fma(mu, v0, b[0]);
                 b[2] = fma(mu, v1, b[2]);
             } else {
@@ -489,7 +512,7 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
                 }
                 else if (P.bc_right == OCI_BC_REFLECTIVE) {
                     v0 = self[(g * N + (N - 1 - m)) * 4 + 1]; v1 = self[(g * N + (N - 1 - m)) * 4 + 3];
-                } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = P.inc_right[gm * 2]; v1 = P.inc_right[gm * 2 + 1]; }
+                } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = incr_s[gm * 2]; v1 = incr_s[gm * 2 + 1]; }
                 b[1] = fma(-mu, v0, b[1]);
                 b[3] = fma(-mu, v1, b[3]);
             }
@@ -499,9 +522,9 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
                            fma(Lp[(p * 4 + 2) * GN], b[2], fma(Lp[(p * 4 + 1) * GN], b[1], Lp[(p * 4) * GN] * b[0])));
         }
         // phi_z = V^T z: the N ordinates of a (cell, group) are N consecutive lanes -> butterfly when N is a power of two
+        double q[4];
         {
             const double wm = on ? w_s[m] : 0.0;
-            double q[4];
 #pragma unroll
             for (int p = 0; p < 4; ++p) q[p] = on ? wm * z[p] : 0.0;
             if (shfl_reduce) {
@@ -519,6 +542,74 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
                 dst[0] = make_double2(q[0], q[1]);
                 dst[1] = make_double2(q[2], q[3]);
             }
+        }
+        if (wl) {
+            // ================= warp-local steps: y = C^-1 phi_z = phi^(l+1), residual, s = dx/4 K y, x = z + D^-1 U y =========
+            double s4[4] = {0.0, 0.0, 0.0, 0.0};
+            if (GC == 1) {
+                if (on) {
+                    const double2 *C2 = reinterpret_cast<const double2 *>(base + lay.Ci + (size_t)a * 16);
+                    double y[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                    for (int cc = 0; cc < 4; ++cc) { // column cc of the column-major 4 x 4 C^-1
+                        const double2 c01 = C2[2 * cc], c23 = C2[2 * cc + 1];
+                        y[0] = fma(c01.x, q[cc], y[0]); y[1] = fma(c01.y, q[cc], y[1]);
+                        y[2] = fma(c23.x, q[cc], y[2]); y[3] = fma(c23.y, q[cc], y[3]);
+                    }
+                    if (gm < 4) {
+                        const double yv = gm == 0 ? y[0] : (gm == 1 ? y[1] : (gm == 2 ? y[2] : y[3]));
+                        P.phi[(size_t)j * 4 + gm] = yv;
+                        const double d = fabs(yv - phi_old);
+                        rmax = (d > rmax || !(d == d)) ? d : rmax;
+                    }
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) { double acc = 0.0; acc = fma(Kr[0], y[p], acc); s4[p] = dxq * 0.25 * acc; }
+                }
+            } else { // (phi_z of the cell's groups was written by the m == 0 lanes above)
+                __syncwarp();
+                if (on && gm < G4) {
+                    const double *Cp = base + lay.Ci + (size_t)a * G4 * G4 + gm;
+                    const double *pz = phiz + a * G4;
+                    double y = 0.0;
+                    for (int cc = 0; cc < G4; ++cc) y = fma(Cp[cc * G4], pz[cc], y);
+                    ys[a * G4 + gm] = y;
+                    P.phi[(size_t)j * G4 + gm] = y;
+                    const double d = fabs(y - phi_old);
+                    rmax = (d > rmax || !(d == d)) ? d : rmax;
+                }
+                __syncwarp();
+                if (on && gm < G4) {
+                    const double *yy = ys + a * G4 + (gm & 3);
+                    double acc = 0.0;
+#pragma unroll
+                    for (int gc = 0; gc < (GC > 0 ? GC : 1); ++gc) acc = fma(Kr[gc], yy[gc * 4], acc);
+                    ss[a * G4 + gm] = dxq * 0.25 * acc;
+                }
+                __syncwarp();
+                if (on) {
+                    const double *sv = ss + a * G4 + g * 4;
+                    s4[0] = sv[0]; s4[1] = sv[1]; s4[2] = sv[2]; s4[3] = sv[3];
+                }
+            }
+            if (on) {
+                double x[4];
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+                    x[p] = fma(Lp[(p * 4 + 3) * GN], s4[3],
+                               fma(Lp[(p * 4 + 2) * GN], s4[2], fma(Lp[(p * 4 + 1) * GN], s4[1], fma(Lp[(p * 4) * GN], s4[0], z[p]))));
+                if (WANT_L2) {
+                    const double *old = base + lay.nb + (size_t)(a + 1) * n + gm * 4;
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) { const double d = x[p] - old[p]; l2 = fma(d, d, l2); }
+                }
+                double *out = P.psi_new + (size_t)j * n + gm * 4;
+                *reinterpret_cast<double2 *>(out) = make_double2(x[0], x[1]);
+                *reinterpret_cast<double2 *>(out + 2) = make_double2(x[2], x[3]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]); // this warp is done with the stage
+            if (++st == stages) { st = 0; ph ^= 1; }
+            continue;
         }
         consumer_sync();
         for (int t2 = tid; !shfl_reduce && t2 < rows; t2 += STP_CONSUMERS) {
@@ -629,11 +720,14 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
                                                                   // falls through when the ring would not fit
         // 256 consumer threads and two CTAs per SM; 128 and four when a cell takes a whole warp (measured: config 3,
         // G N = 32, 16.5 -> 13.4 us per iteration; config 5, G N = 16, is faster with 256: 45 against 47 us)
-        const int CT = (GN > 16 && GN <= 32 && ctx->opt_ctas_per_sm != 2) ? 128 : 256, CPB = CT / GN;
+        const int CT = ctx->opt_st_ct == 128 || ctx->opt_st_ct == 256
+                           ? ctx->opt_st_ct
+                           : ((GN > 16 && GN <= 32 && ctx->opt_ctas_per_sm != 2) ? 128 : 256);
+        const int CPB = CT / GN;
         const int max_ctas = CT == 128 ? 4 : 2;
         const StStage lay = st_stage_layout(ctx->N, ctx->G, CT);
         const size_t fixed = (size_t)2 * STP_MAX_STAGES * 8 + sizeof(double) * ((size_t)2 * ctx->N + (size_t)CPB * GN * 4 +
-                                                                               (size_t)3 * CPB * G4) + 256;
+                                                                               (size_t)3 * CPB * G4 + (size_t)4 * GN) + 256;
         // two CTAs per SM by default: each is a lock-step sequence of short latency-bound phases, two of them overlap
         int ctas = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : max_ctas;
         if (ctas > max_ctas) ctas = max_ctas;
@@ -647,6 +741,9 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
         if (stages > STP_MAX_STAGES) stages = STP_MAX_STAGES;
         if (ctx->opt_stages > 0 && ctx->opt_stages < stages) stages = ctx->opt_stages;
         if (stages >= 2) {
+            // every exchange of a batch inside one warp: N a power of two >= 4, a cell's G N threads do not straddle warps
+            const int warp_local = (ctx->opt_st_warp_local != 0 && (ctx->G == 1 || ctx->G == 2 || ctx->G == 4 || ctx->G == 8) &&
+                                    ctx->N >= 4 && (ctx->N & (ctx->N - 1)) == 0 && GN <= 32) ? 1 : 0;
             const size_t smem = fixed + (size_t)stages * lay.doubles * 8;
             int grid = ctx->num_sms * ctas;
             if (grid > (ctx->J + CPB - 1) / CPB) grid = (ctx->J + CPB - 1) / CPB;
@@ -655,7 +752,7 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
         OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_STP + (((GC_ == 0 ? 0 : (GC_ == 1 ? 1 : (GC_ == 2 ? 2 : (GC_ == 4 ? 3 : 4)))) * 2 + \
                                                       (CT_ == 128 ? 0 : 1)) * 2 + (L2_ ? 1 : 0)),                  \
                                      (const void *)st_iterate_pipe_kernel<L2_, GC_, CT_>, smem));                  \
-        st_iterate_pipe_kernel<L2_, GC_, CT_><<<grid, CT_ + 32, smem, ctx->stream>>>(P, S, stages);                \
+        st_iterate_pipe_kernel<L2_, GC_, CT_><<<grid, CT_ + 32, smem, ctx->stream>>>(P, S, stages, warp_local);    \
     } while (0)
 #define OCI_STP_G(GC_)                                                                                             \
     do {                                                                                                           \
