@@ -330,6 +330,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     ctx->opt_factor_update = 1;
     ctx->opt_persistent = -1;
     ctx->opt_st_warp_local = 1;
+    ctx->opt_st_fused_setup = 1;
     g_create_cuda_error = 0;
     auto fail = [&](int code) { // keeps the CUDA error retrievable: oci_last_create_error()
         if (code == OCI_E_CUDA) {
@@ -430,6 +431,7 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
         ctx->opt_ordering = (int)value;
     }
     else if (!strcmp(key, "st_consumer_threads")) ctx->opt_st_ct = (int)value; // structured pipeline: 128 / 256, 0 = auto
+    else if (!strcmp(key, "st_fused_setup")) { ctx->opt_st_fused_setup = (int)value; if (ctx->opt_solve_mode == 1) ctx->factored = false; }
     else if (!strcmp(key, "st_warp_local")) ctx->opt_st_warp_local = (int)value; // structured pipeline: 0 = CTA barriers
     else if (!strcmp(key, "persistent")) ctx->opt_persistent = (int)value; // -1 auto, 0 off, 1 on (structured path)
     else if (!strcmp(key, "si_sweep")) {

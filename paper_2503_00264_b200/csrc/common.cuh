@@ -78,7 +78,7 @@ struct oci_ctx {
 
     bool factored, c_valid, si_valid, phi_valid;
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering, opt_st_warp_local, opt_st_ct;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering, opt_st_warp_local, opt_st_ct, opt_st_fused_setup;
     // largest dynamic shared-memory size already granted (cudaFuncSetAttribute) to each kernel this context launches;
     // kept per context (= per device), never in function-local statics
     size_t smem_granted[OCI_SMEM_SLOTS];
@@ -316,8 +316,10 @@ __device__ __forceinline__ double lc_entry(int p, int pp, double dx, double sig,
     }
 }
 // ---- 4x4 inverse by Gauss-Jordan with partial pivoting, fully unrolled (registers only) ---------------------
-__device__ __forceinline__ void inv4(double (&a)[4][4], double (&b)[4][4])
+// Returns false if a pivot was zero or not finite (the result is then meaningless).
+__device__ __forceinline__ bool inv4(double (&a)[4][4], double (&b)[4][4])
 {
+    bool ok = true;
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -340,6 +342,7 @@ __device__ __forceinline__ void inv4(double (&a)[4][4], double (&b)[4][4])
                     t = b[k][j]; b[k][j] = b[i][j]; b[i][j] = t;
                 }
             }
+        ok = ok && fabs(a[k][k]) > 0.0 && fabs(a[k][k]) <= 1.7e308; // (NaN fails both)
         const double inv = 1.0 / a[k][k];
 #pragma unroll
         for (int j = 0; j < 4; ++j) { a[k][j] *= inv; b[k][j] *= inv; }
@@ -351,6 +354,7 @@ __device__ __forceinline__ void inv4(double (&a)[4][4], double (&b)[4][4])
                 for (int j = 0; j < 4; ++j) { a[i][j] = fma(-f, a[k][j], a[i][j]); b[i][j] = fma(-f, b[k][j], b[i][j]); }
             }
     }
+    return ok;
 }
 
 #endif

@@ -55,6 +55,66 @@ __global__ void st_wsum_kernel(ProblemView P, const double *__restrict__ LinvT, 
     }
 }
 
+// ---- once per (problem, dt), N a power of two <= 32: st_setup + st_wsum (+ st_cap when G = 1) in ONE launch. One thread
+// per (j,g,m): the block inverse goes to LinvT; W_g = sum_m w_m L^-1 by a butterfly over the N lanes of the (cell, group),
+// which leaves it in every lane; for G = 1 the capacitance matrix C = I - dx/4 K W is 4 x 4 and lane m = 0 inverts it on
+// the spot (round 1: three launches, st_cap with 4 of 32 lanes active and st_wsum reading at stride G N: 0.22 ms on
+// config 5 against 3 x 47 us for the iterations they serve).
+template <bool G1>
+__global__ void __launch_bounds__(256) st_setup_fused_kernel(ProblemView P, double *__restrict__ LinvT, double *__restrict__ Wg,
+                                                             double *__restrict__ Cinv, int *info)
+{
+    const int GN = P.G * P.N, N = P.N;
+    const size_t total = (size_t)P.J * GN;
+    // whole groups of N lanes stay together: the stride is a multiple of 32 and N divides 32
+    for (size_t e0 = (size_t)blockIdx.x * blockDim.x; e0 < total; e0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t e = e0 + threadIdx.x;
+        const bool on = e < total;
+        const size_t ee = on ? e : total - 1;
+        const int gm = (int)(ee % GN), g = gm / N, m = gm - g * N;
+        const size_t j = ee / GN;
+        const double dx = P.dx[j], sig = P.sigma_t[j * P.G + g], v = P.v[g], mu = P.mu[m];
+        double a[4][4], b[4][4];
+#pragma unroll
+        for (int p = 0; p < 4; ++p)
+#pragma unroll
+            for (int pp = 0; pp < 4; ++pp) a[p][pp] = lc_entry(p, pp, dx, sig, v, P.dt, mu);
+        inv4(a, b);
+        if (on) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) LinvT[(j * 16 + k) * GN + gm] = b[k >> 2][k & 3];
+        }
+        const double wm = on ? P.w[m] : 0.0;
+        double ws[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) ws[k] = wm * b[k >> 2][k & 3];
+        for (int o = 1; o < N; o <<= 1) { // butterfly over the ordinates of the (cell, group)
+#pragma unroll
+            for (int k = 0; k < 16; ++k) ws[k] += __shfl_xor_sync(0xffffffffu, ws[k], o);
+        }
+        if (on && m == 0) {
+            double *wo = Wg + (j * P.G + g) * 16;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) wo[k] = ws[k];
+            if (G1) { // C = I - dx/4 K W (4 x 4), inverted with partial pivoting; stored column-major
+                const double k4 = dx * 0.25 * P.transfer[j];
+                double c[4][4], ci[4][4];
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+#pragma unroll
+                    for (int pp = 0; pp < 4; ++pp) c[p][pp] = (p == pp ? 1.0 : 0.0) - k4 * ws[p * 4 + pp];
+                const bool ok = inv4(c, ci);
+                double *out = Cinv + j * 16;
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+#pragma unroll
+                    for (int pp = 0; pp < 4; ++pp) out[pp * 4 + p] = ok ? ci[p][pp] : 0.0;
+                if (!ok) atomicMin(info, (int)j + 1);
+            }
+        }
+    }
+}
+
 // C[(g,p)][(g',p')] = delta - (dx/4 K[g][g']) W_g[p][p']
 __device__ __forceinline__ double cap_entry(const ProblemView &P, const double *__restrict__ Wg, size_t cell, int i, int c)
 {
@@ -696,19 +756,35 @@ int launch_st_factor(oci_ctx *ctx)
     ProblemView P = make_view(ctx);
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream));
     const size_t total = (size_t)ctx->J * ctx->G * ctx->N;
-    size_t g1 = (total + 127) / 128;
-    if (g1 > (size_t)ctx->num_sms * 32) g1 = (size_t)ctx->num_sms * 32;
-    st_setup_kernel<<<(int)g1, 128, 0, ctx->stream>>>(P, ctx->st_LinvT);
-    OCI_CUDA_TRY(ctx, cudaGetLastError());
-    size_t g3 = ((size_t)ctx->J * ctx->G * 16 + 255) / 256;
-    if (g3 > (size_t)ctx->num_sms * 16) g3 = (size_t)ctx->num_sms * 16;
-    st_wsum_kernel<<<(int)g3, 256, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg);
-    OCI_CUDA_TRY(ctx, cudaGetLastError());
+    const bool pow2 = ctx->N <= 32 && (ctx->N & (ctx->N - 1)) == 0;
+    int launches = 0;
+    if (pow2 && ctx->opt_st_fused_setup != 0) {
+        size_t gf = (total + 255) / 256;
+        if (gf > (size_t)ctx->num_sms * 16) gf = (size_t)ctx->num_sms * 16;
+        if (ctx->G == 1) {
+            st_setup_fused_kernel<true><<<(int)gf, 256, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg, ctx->st_Cinv, ctx->info);
+            OCI_CUDA_TRY(ctx, cudaGetLastError());
+            return 1;
+        }
+        st_setup_fused_kernel<false><<<(int)gf, 256, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg, ctx->st_Cinv, ctx->info);
+        OCI_CUDA_TRY(ctx, cudaGetLastError());
+        launches = 1;
+    } else {
+        size_t g1 = (total + 127) / 128;
+        if (g1 > (size_t)ctx->num_sms * 32) g1 = (size_t)ctx->num_sms * 32;
+        st_setup_kernel<<<(int)g1, 128, 0, ctx->stream>>>(P, ctx->st_LinvT);
+        OCI_CUDA_TRY(ctx, cudaGetLastError());
+        size_t g3 = ((size_t)ctx->J * ctx->G * 16 + 255) / 256;
+        if (g3 > (size_t)ctx->num_sms * 16) g3 = (size_t)ctx->num_sms * 16;
+        st_wsum_kernel<<<(int)g3, 256, 0, ctx->stream>>>(P, ctx->st_LinvT, ctx->st_Wg);
+        OCI_CUDA_TRY(ctx, cudaGetLastError());
+        launches = 2;
+    }
     size_t g2 = ((size_t)ctx->J + CAP_WARPS - 1) / CAP_WARPS;
     if (g2 > (size_t)ctx->num_sms * 4) g2 = (size_t)ctx->num_sms * 4;
     st_cap_kernel<<<(int)g2, CAP_WARPS * 32, 0, ctx->stream>>>(P, ctx->st_Wg, ctx->st_Cinv, ctx->info);
     OCI_CUDA_TRY(ctx, cudaGetLastError());
-    return 3;
+    return launches + 1;
 }
 
 int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
