@@ -274,7 +274,8 @@ def run_ours(args):
         for i in range(Wm, Wm + K):
             t = time.perf_counter()
             it, conv, _ = oci_step(i)
-            el = (time.perf_counter() - t) * 1e3   # oci_step is synchronous: host time of the call = its device time + launch gaps
+            oci.synchronize()                      # (the advance kernel may still be in flight when oci_step returns)
+            el = (time.perf_counter() - t) * 1e3   # host time of the call = its device time + launch gaps
             kms, ln = oci.last_timing(1)
             fms, _ = oci.last_timing(0)
             d = per_dt[SWEEP[i % len(SWEEP)]]
@@ -299,6 +300,7 @@ def run_ours(args):
     for i in range(Wm, Wm + K):
         t = time.perf_counter()
         it, conv, _ = oci_step(i, st)
+        st.synchronize()
         el = (time.perf_counter() - t) * 1e3
         d = per_dt[SWEEP[i % len(SWEEP)]]
         d.setdefault("st_iters", []).append(it); d.setdefault("st_ms", []).append(el)
@@ -318,6 +320,7 @@ def run_ours(args):
         si.set_dt(dt)
         torch.cuda.synchronize(); t = time.perf_counter()
         it, conv, _ = si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+        si.synchronize()
         el = (time.perf_counter() - t) * 1e3
         per_dt[dt].setdefault("si_iters", []).append(it)
         per_dt[dt].setdefault("si_ms", []).append(el)
@@ -330,6 +333,7 @@ def run_ours(args):
             si2.set_dt(dt)
             torch.cuda.synchronize(); t = time.perf_counter()
             si2.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)
+            si2.synchronize()
             if i >= Wm:
                 per_dt[dt].setdefault("si_scan_ms", []).append((time.perf_counter() - t) * 1e3)
         del si2
@@ -498,6 +502,7 @@ def run_per_config(device, peak):
                 sol.set_source(p.source_at_step(st))
                 torch.cuda.synchronize(); t = time.perf_counter()
                 it, conv, _ = (sol.step if scheme == 0 else sol.si_step)(tol=p.tol, max_iters=20000, check_every=CHECK_EVERY)
+                sol.synchronize()
                 ms.append((time.perf_counter() - t) * 1e3)
                 iters.append(it)
                 kms.append(sol.last_timing(1 if scheme == 0 else 2)[0])
@@ -552,6 +557,7 @@ def run_as_specified(p, device, no_si):
         oci.set_dt(dt)
         torch.cuda.synchronize(); t = time.perf_counter()
         its = [oci.step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)[0] for _ in range(p.n_steps)]
+        oci.synchronize()
         row["oci_ms_total"] = (time.perf_counter() - t) * 1e3
         row["oci_iters"] = its
         row["oci_ms_per_step"] = row["oci_ms_total"] / p.n_steps
@@ -560,6 +566,7 @@ def run_as_specified(p, device, no_si):
             si.set_dt(dt)
             torch.cuda.synchronize(); t = time.perf_counter()
             its = [si.si_step(tol=TOL, max_iters=MAX_ITERS, check_every=CHECK_EVERY)[0] for _ in range(p.n_steps)]
+            si.synchronize()
             row["si_ms_per_step"] = (time.perf_counter() - t) * 1e3 / p.n_steps
             row["si_iters"] = its
         rows.append(row)

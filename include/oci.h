@@ -137,7 +137,8 @@ int oci_iterate(oci_ctx *ctx, int32_t n_iters);
  * once the rule held, so exactly the natural number of iterations runs; the host reads the residuals and the
  * executed-iterations counter once per batch (the only host round-trip).
  * iters_out[0] = iterations performed, iters_out[1] = iterations after which the rule first held (0 if never);
- * resid_out = last tested residual. Either may be NULL. [sync] */
+ * resid_out = last tested residual. Either may be NULL. [sync] up to the last residual read; the advance kernel may
+ * still be in flight on the stream when the call returns (whatever the caller enqueues next on it is ordered after). */
 int oci_step(oci_ctx *ctx, double tol, int32_t max_iters, int32_t check_every, int32_t stop_rule,
              int32_t advance, int32_t *iters_out, double *resid_out);
 

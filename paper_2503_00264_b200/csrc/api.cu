@@ -176,6 +176,34 @@ bool rule_holds(int rule, double tol, const double *h_inf, const double *h_l2, i
     return e < tol * (1.0 - e / ep);
 }
 
+// a1 + a2 enqueued without a host round-trip: the kernels, their event pair and the copy of the singular-cell flag into
+// pinned memory. factor_finish() reads the flag and the time once the stream has been synchronised (by oci_factor at
+// once, by a step together with its first batch of iterations: one synchronisation instead of two).
+int *factor_info_host(oci_ctx *ctx) { return reinterpret_cast<int *>(ctx->h_resid + 2 * OCI_RESID_CAP + 1); }
+
+int factor_enqueue(oci_ctx *ctx)
+{
+    NvtxRange range(ctx->opt_solve_mode == 1 ? "oci_factor (structured)" : "oci_factor (dense)");
+    OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->evf0, ctx->stream));
+    int r = ctx->opt_solve_mode == 1 ? launch_st_factor(ctx) : launch_factor(ctx);
+    if (r < 0) return r;
+    OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->evf1, ctx->stream));
+    OCI_CUDA_TRY(ctx, cudaMemcpyAsync(factor_info_host(ctx), ctx->info, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->last_launches[0] = r;
+    return 0;
+}
+
+int factor_finish(oci_ctx *ctx)
+{
+    float ms = 0.f;
+    OCI_CUDA_TRY(ctx, cudaEventElapsedTime(&ms, ctx->evf0, ctx->evf1));
+    ctx->last_ms[0] = ms;
+    const int info = *factor_info_host(ctx);
+    if (info != 0x7f7f7f7f) return info; // 1-based index of the first singular cell
+    ctx->factored = true;
+    return 0;
+}
+
 int iterate_impl(oci_ctx *ctx, int scheme, int n_iters)
 {
     if (!ctx) return -1;
@@ -219,10 +247,12 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
         if (scheme == 0) ctx->factored = false;
         else ctx->si_valid = false;
     }
+    bool factor_pending = false;
     if (scheme == 0) {
-        if (!ctx->factored) {
-            if ((r = oci_factor(ctx)) != 0) return r;
+        if (!ctx->factored) { // enqueued here, checked with the first batch's read-back below
+            if ((r = factor_enqueue(ctx)) < 0) return r;
             launches += ctx->last_launches[0];
+            factor_pending = true;
         }
         if ((r = ensure_const_rhs(ctx, &launches)) < 0) return r;
     } else {
@@ -255,6 +285,10 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
                                               ctx->stream));
         OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_exec, ctx->ctrl, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        if (factor_pending) { // a singular cell: the iterations of this batch ran on a zeroed block; report it
+            factor_pending = false;
+            if ((r = factor_finish(ctx)) != 0) return r;
+        }
         {
             float t = 0.f; // device time of this batch of k launches (kernels only, no flag read)
             OCI_CUDA_TRY(ctx, cudaEventElapsedTime(&t, ctx->ev0, ctx->ev1));
@@ -279,7 +313,7 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
         ctx->last_launches[which] += r;
         ctx->c_valid = false;
     }
-    OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    // (no synchronisation here: the advance kernel is stream-ordered before anything the caller enqueues next)
     if (iters_out) { iters_out[0] = it; iters_out[1] = conv_at; }
     if (resid_out) *resid_out = last;
     return 0;
@@ -351,9 +385,10 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     device_limits(&ctx->num_sms, &ctx->max_smem_optin, ctx->device);
     const size_t need = carve(ctx, (unsigned char *)workspace_dev, p->J, p->N, p->G, ctx->num_sms, ctx->max_smem_optin);
     if (need > workspace_bytes) return fail(OCI_E_WORKSPACE);
-    if (cudaHostAlloc((void **)&ctx->h_resid, sizeof(double) * (2 * OCI_RESID_CAP + 2), cudaHostAllocDefault) != cudaSuccess)
+    if (cudaHostAlloc((void **)&ctx->h_resid, sizeof(double) * (2 * OCI_RESID_CAP + 4), cudaHostAllocDefault) != cudaSuccess)
         return fail(OCI_E_CUDA);
     if (cudaEventCreate(&ctx->ev0) != cudaSuccess || cudaEventCreate(&ctx->ev1) != cudaSuccess) return fail(OCI_E_CUDA);
+    if (cudaEventCreate(&ctx->evf0) != cudaSuccess || cudaEventCreate(&ctx->evf1) != cudaSuccess) return fail(OCI_E_CUDA);
     cudaStream_t s = ctx->stream;
     const size_t J = p->J, G = p->G, N = p->N, n = ctx->n;
 #define UP(dst, src, cnt)                                                                                      \
@@ -390,6 +425,8 @@ void oci_destroy(oci_ctx *ctx)
     if (ctx->h_resid) cudaFreeHost(ctx->h_resid);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    if (ctx->evf0) cudaEventDestroy(ctx->evf0);
+    if (ctx->evf1) cudaEventDestroy(ctx->evf1);
     delete ctx;
 }
 
@@ -520,21 +557,10 @@ int oci_factor(oci_ctx *ctx)
     if (!ctx) return -1;
     DeviceGuard guard(ctx->device);
     if (ctx->factored) return 0;
-    NvtxRange range(ctx->opt_solve_mode == 1 ? "oci_factor (structured)" : "oci_factor (dense)");
-    OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
-    int r = ctx->opt_solve_mode == 1 ? launch_st_factor(ctx) : launch_factor(ctx);
+    int r = factor_enqueue(ctx);
     if (r < 0) return r;
-    OCI_CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
-    int info = 0;
-    OCI_CUDA_TRY(ctx, cudaMemcpyAsync(&info, ctx->info, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
-    float ms = 0.f;
-    OCI_CUDA_TRY(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
-    ctx->last_ms[0] = ms;
-    ctx->last_launches[0] = r;
-    if (info != 0x7f7f7f7f) return info; // 1-based index of the first singular cell
-    ctx->factored = true;
-    return 0;
+    return factor_finish(ctx);
 }
 
 int oci_iterate(oci_ctx *ctx, int32_t n_iters)

@@ -84,6 +84,7 @@ struct oci_ctx {
     size_t smem_granted[OCI_SMEM_SLOTS];
     // timing
     cudaEvent_t ev0, ev1;
+    cudaEvent_t evf0, evf1;        // bracket the factor launch (own pair: a step enqueues factor + iterations before it syncs)
     double last_ms[3];
     long long last_launches[3];
 };
