@@ -98,9 +98,9 @@ def ncu_traffic(kernel: str, workload: str):
 
 
 def structured_bytes_per_cell_solve(n: int, G: int) -> int:
-    """DESIGN.md section 5 (structured cell solve): L^-1 blocks (32 n) + c (8n) + neighbour edge flux
-    (4n) + Psi write (8n) + C^-1 (128 G^2) + K (8 G^2) + dx (8) + phi read/write (64 G)."""
-    return 52 * n + 136 * G * G + 64 * G + 8
+    """DESIGN.md section 5 (structured cell solve): L^-1 blocks, two of their four rows (16 n) + c (8n)
+    + neighbour edge flux (4n) + Psi write (8n) + C^-1 (128 G^2) + K (8 G^2) + dx (8) + phi read/write (64 G)."""
+    return 36 * n + 136 * G * G + 64 * G + 8
 
 
 def algorithmic_bytes_per_cell_solve(n: int, G: int) -> int:

@@ -99,7 +99,7 @@ size_t carve(oci_ctx *c, unsigned char *base, int J, int N, int G, int num_sms, 
     // scan mode: 6 doubles per thread prefix (one thread per 4 sweep steps) + per 1024-step block aggregate, per chain
     t->si_scan_bytes = (((size_t)J + 1023) / 1024) * GN * 257 * 6 * sizeof(double);
     t->si_scan = cv.take<double>(t->si_scan_bytes / sizeof(double));
-    t->st_LinvT = cv.take<double>((size_t)J * GN * 16);
+    t->st_LinvT = cv.take<double>((size_t)J * GN * 8); // two of the four rows of every block inverse (structured.cu ST_LK)
     t->st_Wg = cv.take<double>((size_t)J * G * 16);
     t->st_Cinv = cv.take<double>((size_t)J * 16 * G * G);
     t->resid_inf = cv.take<unsigned long long>(OCI_RESID_CAP);

@@ -62,7 +62,7 @@ struct oci_ctx {
     double *si_scan;    // scan mode ("si_sweep" = 1): per-thread prefixes and per-block aggregates (si.cu)
     size_t si_scan_bytes;
     // structured cell solve ("solve_mode" = 1; structured.cu)
-    double *st_LinvT;   // [J][16][G*N]   L_{c,j,g,m}^-1, ordinate-fastest
+    double *st_LinvT;   // [J][8][G*N]    rows (k,L), (k+1/2,L) of L_{c,j,g,m}^-1, ordinate-fastest (structured.cu ST_LK)
     double *st_Wg;      // [J][G][16]     sum_m w_m L^-1_{j,g,m}
     double *st_Cinv;    // [J][4G(col)][4G(row)]  (I - V^T D^-1 U)^-1, column-major per cell
     // residual history (device) + pinned host mirror

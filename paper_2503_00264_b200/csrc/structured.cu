@@ -17,8 +17,23 @@
 
 namespace {
 
-// ---- once per (problem, dt): LinvT[j][k][gm] = (L_{c,j,g,m}^-1)[k/4][k%4] (ordinate-fastest, so that the iterate
-// kernel's loads and these stores are contiguous across threads). One thread per (j,g,m).
+// The block L_{c,j,g,m} of Eq. 8b is a 2 x 2 matrix over the numbers x + y J, J = [[0, 1], [-1, 0]] (J^2 = -I):
+//     L = [[alpha, gamma/2], [-gamma, alpha + gamma]],  alpha = a I + (mu/2) J,
+// and so is its inverse: every 2 x 2 sub-block of L^-1 has the form [[x, y], [-y, x]]. Rows (k,R) and (k+1/2,R) of L^-1
+// therefore follow from rows (k,L) and (k+1/2,L), and only those two rows are stored and streamed: ST_LK = 8 doubles
+// per block instead of 16 (the largest item of the structured path's traffic, halved). stored[0..3] = row 0,
+// stored[4..7] = row 2 of the inverse inv4() computes with partial pivoting.
+constexpr int ST_LK = 8;
+// entry (p, c) of L^-1 from the stored rows (p, c compile-time constants in every use)
+__device__ __forceinline__ double st_L(const double (&s)[ST_LK], int p, int c)
+{
+    const int r = (p >> 1) * 4;
+    if (!(p & 1)) return s[r + c];
+    return (c & 1) ? s[r + c - 1] : -s[r + c + 1];
+}
+
+// ---- once per (problem, dt): LinvT[j][k][gm], k < ST_LK (ordinate-fastest, so that the iterate kernel's loads and these
+// stores are contiguous across threads). One thread per (j,g,m).
 __global__ void st_setup_kernel(ProblemView P, double *__restrict__ LinvT)
 {
     const int GN = P.G * P.N;
@@ -34,7 +49,7 @@ __global__ void st_setup_kernel(ProblemView P, double *__restrict__ LinvT)
             for (int pp = 0; pp < 4; ++pp) a[p][pp] = lc_entry(p, pp, dx, sig, v, P.dt, mu);
         inv4(a, b);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) LinvT[(j * 16 + k) * GN + gm] = b[k >> 2][k & 3];
+        for (int k = 0; k < ST_LK; ++k) LinvT[(j * ST_LK + k) * GN + gm] = b[(k >> 2) * 2][k & 3];
     }
 }
 
@@ -44,14 +59,17 @@ __global__ void st_wsum_kernel(ProblemView P, const double *__restrict__ LinvT, 
     const int GN = P.G * P.N;
     const size_t total = (size_t)P.J * P.G * 16;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (size_t)gridDim.x * blockDim.x) {
-        const int k = (int)(e & 15);
+        const int k = (int)(e & 15), p = k >> 2, c = k & 3;
         const size_t jg = e >> 4;
         const int g = (int)(jg % P.G);
         const size_t j = jg / P.G;
-        const double *src = LinvT + (j * 16 + k) * GN + (size_t)g * P.N;
+        // entry (p, c) of L^-1 = +- a stored entry (see st_L)
+        const int ks = (p >> 1) * 4 + ((p & 1) ? ((c & 1) ? c - 1 : c + 1) : c);
+        const double sgn = ((p & 1) && !(c & 1)) ? -1.0 : 1.0;
+        const double *src = LinvT + (j * ST_LK + ks) * GN + (size_t)g * P.N;
         double acc = 0.0;
         for (int m = 0; m < P.N; ++m) acc = fma(P.w[m], src[m], acc);
-        Wg[e] = acc;
+        Wg[e] = sgn * acc;
     }
 }
 
@@ -80,14 +98,17 @@ __global__ void __launch_bounds__(256) st_setup_fused_kernel(ProblemView P, doub
 #pragma unroll
             for (int pp = 0; pp < 4; ++pp) a[p][pp] = lc_entry(p, pp, dx, sig, v, P.dt, mu);
         inv4(a, b);
+        double st[ST_LK];
+#pragma unroll
+        for (int k = 0; k < ST_LK; ++k) st[k] = b[(k >> 2) * 2][k & 3];
         if (on) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) LinvT[(j * 16 + k) * GN + gm] = b[k >> 2][k & 3];
+            for (int k = 0; k < ST_LK; ++k) LinvT[(j * ST_LK + k) * GN + gm] = st[k];
         }
         const double wm = on ? P.w[m] : 0.0;
         double ws[16];
 #pragma unroll
-        for (int k = 0; k < 16; ++k) ws[k] = wm * b[k >> 2][k & 3];
+        for (int k = 0; k < 16; ++k) ws[k] = wm * st_L(st, k >> 2, k & 3); // the block as the iterate kernels will see it
         for (int o = 1; o < N; o <<= 1) { // butterfly over the ordinates of the (cell, group)
 #pragma unroll
             for (int k = 0; k < 16; ++k) ws[k] += __shfl_xor_sync(0xffffffffu, ws[k], o);
@@ -223,7 +244,7 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
     for (int base = blockIdx.x * CPB; base < Jc; base += gridDim.x * CPB) {
         const int j = NC * (base + a) + P.color;
         const bool on = lane_on && base + a < Jc;
-        double L[16], z[4], b[4], v0 = 0.0, v1 = 0.0, mu = 1.0;
+        double L[ST_LK], z[4], b[4], v0 = 0.0, v1 = 0.0, mu = 1.0;
         // ---- all global loads of this batch up front
         if (on) {
             const double2 c01 = *reinterpret_cast<const double2 *>(P.c + (size_t)j * n + gm * 4);
@@ -243,9 +264,9 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
                     v0 = ld_iter<COHERENT>(self + (g * N + (N - 1 - m)) * 4 + 1); v1 = ld_iter<COHERENT>(self + (g * N + (N - 1 - m)) * 4 + 3);
                 } else if (P.bc_right == OCI_BC_PRESCRIBED) { v0 = P.inc_right[gm * 2]; v1 = P.inc_right[gm * 2 + 1]; }
             }
-            const double *Lp = S.LinvT + (size_t)j * 16 * GN + gm;
+            const double *Lp = S.LinvT + (size_t)j * ST_LK * GN + gm;
 #pragma unroll
-            for (int k = 0; k < 16; ++k) L[k] = Lp[(size_t)k * GN];
+            for (int k = 0; k < ST_LK; ++k) L[k] = Lp[(size_t)k * GN];
         }
         double Cr[4 * GP], Kr[GP], dxq = 0.0, phi_old = 0.0; // this thread's (first) row of the 4G-system
         if (PRE && tid < rows && base + tid / G4 < Jc) {
@@ -266,7 +287,7 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
             const double wm = w_s[m];
 #pragma unroll
             for (int p = 0; p < 4; ++p) { // z = D^-1 b
-                z[p] = fma(L[p * 4 + 3], b[3], fma(L[p * 4 + 2], b[2], fma(L[p * 4 + 1], b[1], L[p * 4] * b[0])));
+                z[p] = fma(st_L(L, p, 3), b[3], fma(st_L(L, p, 2), b[2], fma(st_L(L, p, 1), b[1], st_L(L, p, 0) * b[0])));
                 wz[(size_t)tid * 4 + p] = wm * z[p];
             }
         }
@@ -330,7 +351,7 @@ __device__ __forceinline__ void st_iterate_body(const IterParams &P, const StPar
             double x[4];
 #pragma unroll
             for (int p = 0; p < 4; ++p)
-                x[p] = fma(L[p * 4 + 3], s3, fma(L[p * 4 + 2], s2, fma(L[p * 4 + 1], s1, fma(L[p * 4], s0, z[p]))));
+                x[p] = fma(st_L(L, p, 3), s3, fma(st_L(L, p, 2), s2, fma(st_L(L, p, 1), s1, fma(st_L(L, p, 0), s0, z[p]))));
             double *out = P.psi_new + (size_t)j * n + gm * 4;
             if (WANT_L2) {
                 const double *old = P.psi_old + (size_t)j * n + gm * 4;
@@ -418,7 +439,7 @@ __host__ __device__ inline StStage st_stage_layout(int N, int G, int CT)
     const int GN = G * N, n = 4 * GN, G4 = 4 * G, CPB = CT / GN;
     StStage s;
     s.Lt = 0;
-    s.cs = s.Lt + CPB * 16 * GN;
+    s.cs = s.Lt + CPB * ST_LK * GN;
     s.nb = s.cs + CPB * n;
     s.Ci = s.nb + (CPB + 2) * n;
     s.doubles = (s.Ci + CPB * G4 * G4 + 15) & ~15; // stages stay 128-byte aligned
@@ -478,12 +499,12 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
                 mbar_wait(&empty[st], ph ^ 1);
                 double *base = ring + (size_t)st * lay.doubles;
                 const int lo = max(gb - 1, 0), hi = min(gb + nb, J - 1);
-                const uint32_t bL = (uint32_t)((size_t)nb * 16 * GN * sizeof(double));
+                const uint32_t bL = (uint32_t)((size_t)nb * ST_LK * GN * sizeof(double));
                 const uint32_t bc = (uint32_t)((size_t)nb * n * sizeof(double));
                 const uint32_t bn = (uint32_t)((size_t)(hi - lo + 1) * n * sizeof(double));
                 const uint32_t bC = (uint32_t)((size_t)nb * G4 * G4 * sizeof(double));
                 mbar_arrive_expect_tx(&full[st], bL + bc + bn + bC);
-                bulk_g2s(base + lay.Lt, S.LinvT + (size_t)gb * 16 * GN, bL, &full[st]);
+                bulk_g2s(base + lay.Lt, S.LinvT + (size_t)gb * ST_LK * GN, bL, &full[st]);
                 bulk_g2s(base + lay.cs, P.c + (size_t)gb * n, bc, &full[st]);
                 bulk_g2s(base + lay.nb + (size_t)(lo - (gb - 1)) * n, P.psi_old + (size_t)lo * n, bn, &full[st]);
                 bulk_g2s(base + lay.Ci, S.Cinv + (size_t)gb * G4 * G4, bC, &full[st]);
@@ -546,7 +567,21 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
         load_role2(gb + CPB, min(CPB, cell1 - gb - CPB));
         mbar_wait(&full[st], ph);
         double z[4];
-        const double *Lp = base + lay.Lt + (size_t)a * 16 * GN + gm;
+        // the two stored rows of this thread's block inverse: in registers, except for G = 8, whose instantiation has
+        // none to spare (it re-reads them from the stage)
+        constexpr bool L_IN_REGS = GC != 8;
+        const double *Lp = base + lay.Lt + (size_t)a * ST_LK * GN + gm;
+        double Ls[ST_LK];
+        if (L_IN_REGS) {
+#pragma unroll
+            for (int k = 0; k < ST_LK; ++k) Ls[k] = on ? Lp[k * GN] : 0.0;
+        }
+        auto Lent = [&](int p, int c) -> double {
+            if (L_IN_REGS) return st_L(Ls, p, c);
+            const int r = (p >> 1) * 4;
+            if (!(p & 1)) return Lp[(r + c) * GN];
+            return (c & 1) ? Lp[(r + c - 1) * GN] : -Lp[(r + c + 1) * GN];
+        };
         if (on) {
             const double2 *cp = reinterpret_cast<const double2 *>(base + lay.cs + (size_t)a * n + gm * 4);
             const double2 c01 = cp[0], c23 = cp[1];
@@ -578,8 +613,7 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
             }
 #pragma unroll
             for (int p = 0; p < 4; ++p) // z = D^-1 b
-                z[p] = fma(Lp[(p * 4 + 3) * GN], b[3],
-                           fma(Lp[(p * 4 + 2) * GN], b[2], fma(Lp[(p * 4 + 1) * GN], b[1], Lp[(p * 4) * GN] * b[0])));
+                z[p] = fma(Lent(p, 3), b[3], fma(Lent(p, 2), b[2], fma(Lent(p, 1), b[1], Lent(p, 0) * b[0])));
         }
         // phi_z = V^T z: the N ordinates of a (cell, group) are N consecutive lanes -> butterfly when N is a power of two
         double q[4];
@@ -655,8 +689,7 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
                 double x[4];
 #pragma unroll
                 for (int p = 0; p < 4; ++p)
-                    x[p] = fma(Lp[(p * 4 + 3) * GN], s4[3],
-                               fma(Lp[(p * 4 + 2) * GN], s4[2], fma(Lp[(p * 4 + 1) * GN], s4[1], fma(Lp[(p * 4) * GN], s4[0], z[p]))));
+                    x[p] = fma(Lent(p, 3), s4[3], fma(Lent(p, 2), s4[2], fma(Lent(p, 1), s4[1], fma(Lent(p, 0), s4[0], z[p]))));
                 if (WANT_L2) {
                     const double *old = base + lay.nb + (size_t)(a + 1) * n + gm * 4;
 #pragma unroll
@@ -722,8 +755,7 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
             double x[4];
 #pragma unroll
             for (int p = 0; p < 4; ++p)
-                x[p] = fma(Lp[(p * 4 + 3) * GN], s3,
-                           fma(Lp[(p * 4 + 2) * GN], s2, fma(Lp[(p * 4 + 1) * GN], s1, fma(Lp[(p * 4) * GN], s0, z[p]))));
+                x[p] = fma(Lent(p, 3), s3, fma(Lent(p, 2), s2, fma(Lent(p, 1), s1, fma(Lent(p, 0), s0, z[p]))));
             if (WANT_L2) {
                 const double *old = base + lay.nb + (size_t)(a + 1) * n + gm * 4;
 #pragma unroll
@@ -890,7 +922,7 @@ int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_bet
 {
     if (ctx->opt_solve_mode != 1 || ctx->opt_persistent == 0 || ctx->opt_ordering != 0 || k < 2) return 0;
     const int GN = ctx->G * ctx->N, CPB = ST_THREADS / GN, G4 = 4 * ctx->G;
-    const size_t bytes_per_iter = (size_t)ctx->J * (52 * (size_t)ctx->n + 136 * (size_t)ctx->G * ctx->G + 64 * ctx->G + 8);
+    const size_t bytes_per_iter = (size_t)ctx->J * (36 * (size_t)ctx->n + 136 * (size_t)ctx->G * ctx->G + 64 * ctx->G + 8);
     if (ctx->opt_persistent < 0 && bytes_per_iter > ((size_t)8 << 20)) return 0;
     int coop = 0;
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess || !coop) return 0;

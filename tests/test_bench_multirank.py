@@ -47,7 +47,7 @@ def test_single_process_helpers_need_no_process_group():
     assert bench.max_over_ranks(4.25, device="cpu") == 4.25
     assert bench.whole_job_value(1, 65536, 20, 10.0) == pytest.approx(65536 * 20 / 0.01)
     assert bench.algorithmic_bytes_per_cell_solve(64, 1) == 8 * 64 * 64 + 24 * 64 + 64
-    assert bench.structured_bytes_per_cell_solve(64, 1) == 52 * 64 + 136 + 64 + 8
+    assert bench.structured_bytes_per_cell_solve(64, 1) == 36 * 64 + 136 + 64 + 8
 
 
 def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
