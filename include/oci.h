@@ -103,9 +103,12 @@ int oci_last_create_error(void);
  * a1+a2 at the start of every step as Alg. 2 prints it; 0 [default] = only when dt changed), "si_lanes" (ordinates x
  * groups swept by one CTA of the SI sweep kernel: 4, 8 [default] or 16), "si_sweep" (0 = serial in space [default],
  * the comparator north_star names; 1 = the same sweep evaluated as a parallel scan of the per-cell affine edge maps,
- * same iterates to rounding), "persistent" (structured path only: -1 [default] = run a batch
- * of iterations as ONE cooperative launch with grid-wide barriers when the problem is small (<= 8 MB per iteration),
- * 0 = never, 1 = always), "ordering" (structured path only: 0 = block-Jacobi [default], the
+ * same iterates to rounding), "persistent" (-1 [default] = run a batch of iterations as ONE
+ * cooperative launch with grid-wide barriers when the problem is small: structured path <= 8 MB per iteration; dense
+ * path when the inverses of ceil(J / SMs) cells fit in one CTA's shared memory, where they then stay for the whole
+ * batch; 0 = never, 1 = always (structured path)), "st_warp_local", "st_consumer_threads",
+ * "st_fused_setup" (structured path, tuning probes: 0 restores the CTA barriers per batch / 128 or 256 consumer
+ * threads per CTA / 0 restores the three set-up launches), "ordering" (structured path only: 0 = block-Jacobi [default], the
  * paper's OCI; 1 = red-black: per iteration the even cells, then the odd cells from the new even ones, in place --
  * the block Gauss-Seidel variant PAPER.md:29, 550 names, about half the iterations; SURVEY.md 8(f) row f4;
  * oci_iterate / oci_step return OCI_E_UNSUPPORTED in the dense mode). Returns -2 for an unknown key, -3 for a bad

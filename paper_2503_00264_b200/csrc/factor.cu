@@ -1038,11 +1038,14 @@ struct P128Shared {
     int cell, sing, tie;
 };
 
-__device__ __forceinline__ void p128_bar_pivot() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+// named barrier over the AW pivot warps of a CTA
+template <int AW> __device__ __forceinline__ void pivot_warps_bar() { asm volatile("bar.sync 1, %0;" ::"n"(32 * AW) : "memory"); }
+__device__ __forceinline__ void p128_bar_pivot() { pivot_warps_bar<P128_AW>(); }
 
-template <int b, bool FAST>
-__device__ __forceinline__ void p128_pivot_step(double (&t)[FR_NB], unsigned &m, P128Shared &sh, int w, int lane, int col0,
-                                                unsigned &bad, unsigned &tie)
+// One pivot step of a panel shared by AW pivot warps, one row per lane (row 32 w + lane). slots: [2][AW].
+template <int b, bool FAST, int AW>
+__device__ __forceinline__ void pw_pivot_step(double (&t)[FR_NB], unsigned &m, P128Slot *slots, int *rho, int *rhoinv, int w,
+                                              int lane, int col0, unsigned &bad, unsigned &tie)
 {
     constexpr unsigned FULL = 0xffffffffu;
     const unsigned h = (unsigned)__double2hiint(t[b]) & m, l = (unsigned)__double2loint(t[b]);
@@ -1056,7 +1059,7 @@ __device__ __forceinline__ void p128_pivot_step(double (&t)[FR_NB], unsigned &m,
         ball = __ballot_sync(FULL, cand && l == ml);
     }
     const int src = (__ffs(ball) - 1) & 31;
-    P128Slot *mine = &sh.slot[b & 1][w];
+    P128Slot *mine = &slots[(b & 1) * AW + w];
     if (lane == src) { // this warp's candidate: key, row as it stands, 1 / candidate
 #pragma unroll
         for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(mine->row)[c] = make_double2(t[2 * c], t[2 * c + 1]);
@@ -1064,30 +1067,30 @@ __device__ __forceinline__ void p128_pivot_step(double (&t)[FR_NB], unsigned &m,
         mine->key = ((unsigned long long)h << 32) | l; // h == 0: no unused row here (loses, or the cell is singular)
         mine->lane = lane | (tied ? 0x100 : 0);
     }
-    p128_bar_pivot();
-    // the four candidates: key and lane word of a slot in one 16-byte broadcast load
-    unsigned long long kk[P128_AW];
-    int lw4[P128_AW];
+    pivot_warps_bar<AW>();
+    // the AW candidates: key and lane word of a slot in one 16-byte broadcast load
+    unsigned long long kk[AW];
+    int lw4[AW];
 #pragma unroll
-    for (int ww = 0; ww < P128_AW; ++ww) {
-        const uint4 v = *reinterpret_cast<const uint4 *>(&sh.slot[b & 1][ww].key);
+    for (int ww = 0; ww < AW; ++ww) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(&slots[(b & 1) * AW + ww].key);
         kk[ww] = ((unsigned long long)v.y << 32) | v.x;
         lw4[ww] = (int)v.z;
     }
     unsigned long long kmax = kk[0];
     int gw = 0, lwv = lw4[0];
 #pragma unroll
-    for (int ww = 1; ww < P128_AW; ++ww) // strict >: a tie goes to the lower warp, i.e. the lower row
+    for (int ww = 1; ww < AW; ++ww) // strict >: a tie goes to the lower warp, i.e. the lower row
         if (kk[ww] > kmax) { kmax = kk[ww]; gw = ww; lwv = lw4[ww]; }
     if (FAST) { // an unresolved tie matters only where it could have hidden the true maximum: in a warp whose published
                 // high word equals the winning one (most warps tie on the identical entries -dx K w / 4 of Eq. 10, far
                 // below the pivot)
 #pragma unroll
-        for (int ww = 0; ww < P128_AW; ++ww)
+        for (int ww = 0; ww < AW; ++ww)
             if ((lw4[ww] & 0x100) && (unsigned)(kk[ww] >> 32) == (unsigned)(kmax >> 32)) tie |= 1u;
     }
     bad |= ((unsigned)(kmax >> 32) - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot
-    const P128Slot *win = &sh.slot[b & 1][gw];
+    const P128Slot *win = &slots[(b & 1) * AW + gw];
     const double ls = win->linv;
     const int lw = lwv & 31;
     double sp[FR_NB];
@@ -1103,23 +1106,23 @@ __device__ __forceinline__ void p128_pivot_step(double (&t)[FR_NB], unsigned &m,
     m = is_p ? 0u : m;
     if (w == 0 && lane == b) {
         const int r = 32 * gw + lw;
-        sh.rho[col0 + b] = r;
-        sh.rhoinv[r] = col0 + b;
+        rho[col0 + b] = r;
+        rhoinv[r] = col0 + b;
     }
 }
 
-template <bool FAST>
-__device__ __forceinline__ void p128_panel(double (&t)[FR_NB], unsigned &m, P128Shared &sh, int w, int lane, int col0,
-                                           unsigned &bad, unsigned &tie)
+template <bool FAST, int AW>
+__device__ __forceinline__ void pw_panel(double (&t)[FR_NB], unsigned &m, P128Slot *slots, int *rho, int *rhoinv, int w, int lane,
+                                         int col0, unsigned &bad, unsigned &tie)
 {
-    p128_pivot_step<0, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<1, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<2, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<3, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<4, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<5, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<6, FAST>(t, m, sh, w, lane, col0, bad, tie);
-    p128_pivot_step<7, FAST>(t, m, sh, w, lane, col0, bad, tie);
+    pw_pivot_step<0, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<1, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<2, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<3, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<4, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<5, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<6, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    pw_pivot_step<7, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
 }
 
 // one whole column block by one warp (see wc2_update_blocks): pivot rows read, zeroed, 16 row tiles updated
@@ -1177,7 +1180,7 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
                 for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
                 unsigned bad = 0u, tie = 0u;
                 const unsigned m_in = m;
-                p128_panel<true>(t, m, sh, w, lane, FR_NB * pnl, bad, tie);
+                pw_panel<true, P128_AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
                 if (tie) sh.tie = 1;
                 p128_bar_pivot();
                 const bool redo = sh.tie != 0;
@@ -1188,7 +1191,7 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
                     for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
                     m = m_in;
                     bad = 0u;
-                    p128_panel<false>(t, m, sh, w, lane, FR_NB * pnl, bad, tie);
+                    pw_panel<false, P128_AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
                 }
                 if (bad && threadIdx.x == 0) sh.sing = 1;
 #pragma unroll
@@ -1255,6 +1258,205 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
         }
         __syncthreads(); // everybody is done with W and sh.cell before the next cell
     }
+}
+
+// ============================================================================================================
+// n = 64 NQ, NQ = 3, 4 (n = 192, 256: config 4, Table 2 with S32): a cluster of NQ CTAs per cell, working matrix in the
+// DISTRIBUTED shared memory of the cluster.
+// ============================================================================================================
+// The design of factor_p128_kernel where one working matrix (532 KB at n = 256) no longer fits one SM: CTA q of the
+// cluster keeps columns [64 q, 64 q + 64) (133 KB, column-major, leading dimension n + 4). Panel p (8 columns) belongs to
+// CTA p / 8: its n / 32 pivot warps (one row per lane) eliminate it out of their own shared memory exactly as in the
+// n = 128 kernel -- nothing in a pivot step leaves the SM. The eliminated panel T (n x 8), the pivot rows R and the
+// singular flag then travel ONCE to every other CTA of the cluster: the owner writes them to its own panel buffer and
+// one thread issues a bulk asynchronous copy (cp.async.bulk shared::cta -> shared::cluster, completion on the
+// receiver's mbarrier) per peer; every CTA then applies the rank-8 update to its own eight column blocks (transposed
+// m8n8k4 DMMAs, pivot rows zeroed, one warp per block) from its local copy. One cluster barrier per panel orders the
+// re-use of the two panel buffers and the hand-over of the pivot role from CTA to CTA.
+constexpr int CQ_THREADS = 384; // 12 warps: the first n / 32 are pivot warps when the CTA owns the panel
+
+template <int NQ> struct CqPanelBuf {
+    double T[FR_NB][64 * NQ + 4]; // [panel column][row]
+    int R[FR_NB];
+    int sing, pad[7];
+};
+
+template <int NQ> struct CqShared {
+    double W[64 * (64 * NQ + 4)];     // [local column][row]
+    CqPanelBuf<NQ> pb[2];             // [panel parity]
+    P128Slot slot[2][2 * NQ];         // [step parity][pivot warp]
+    uint64_t tfull[2];                // panel buffer `parity` holds panel p
+    int rho[64 * NQ], rhoinv[64 * NQ];
+    int tie;
+};
+
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t local_addr, uint32_t cta_rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta_rank));
+    return r;
+}
+__device__ __forceinline__ void bulk_s2peer(uint32_t dst_cluster, const void *src_smem, uint32_t bytes, uint32_t bar_cluster)
+{
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_cluster),
+                 "r"(smem_u32(src_smem)), "r"(bytes), "r"(bar_cluster)
+                 : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+
+template <int NQ, bool DUMP>
+__global__ void __launch_bounds__(CQ_THREADS, 1)
+factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__restrict__ dumpA, int dump_cell)
+{
+    constexpr int n = 64 * NQ, LD = n + 4, NPANEL = n / FR_NB, AW = 2 * NQ, NWARP = CQ_THREADS / 32;
+    extern __shared__ __align__(16) unsigned char cq_smem[];
+    CqShared<NQ> &sh = *reinterpret_cast<CqShared<NQ> *>(cq_smem);
+    double *W = sh.W;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
+    const int q = (int)cluster_ctarank();
+    const int n_clusters = gridDim.x / NQ, cluster_id = blockIdx.x / NQ;
+
+    if (threadIdx.x == 0) {
+        mbar_init(&sh.tfull[0], 1);
+        mbar_init(&sh.tfull[1], 1);
+        fence_mbar_init();
+        sh.tie = 0;
+    }
+    cluster_sync_all(); // barriers initialised everywhere before any peer copies into this CTA
+    unsigned gp = 0;    // panels processed so far by this cluster (selects buffer and barrier parity)
+
+    for (int cell = DUMP ? dump_cell : cluster_id; cell < P.J; cell += n_clusters) {
+        // ---- a1: this CTA's 64 columns (16 column blocks of 4) x n rows
+        {
+            double *Wl = W - (size_t)64 * q * LD; // so that the global column index addresses the local array
+            for (int idx = w; idx < NQ * 16; idx += NWARP)
+                assemble_rows2(P, cell, lane, Wl, LD, 16 * q + (idx & 15), 1 << 20, 64 * (idx >> 4), 1 << 20);
+        }
+        __syncthreads();
+        if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
+            for (int e = threadIdx.x; e < n * 64; e += CQ_THREADS) dumpA[(size_t)(e / 64) * n + 64 * q + (e & 63)] = W[(e & 63) * LD + e / 64];
+            break;
+        }
+
+        unsigned m = 0x7fffffffu; // pivot warps: 0 once row 32 w + lane has been a pivot row (tracked in every CTA)
+        bool singular = false;
+        for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
+            const int owner = pnl >> 3, lb = pnl & 7, buf = gp & 1;
+            const uint32_t par = (gp >> 1) & 1;
+            CqPanelBuf<NQ> &pb = sh.pb[buf];
+            if (q == owner) {
+                if (w < AW) {
+                    // ================= phase P: the owner's pivot warps eliminate the n x 8 panel, one row per lane =========
+                    const int r = 32 * w + lane;
+                    double *Wp = &W[(FR_NB * lb) * LD + r];
+                    double t[FR_NB];
+#pragma unroll
+                    for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
+                    unsigned bad = 0u, tie = 0u;
+                    const unsigned m_in = m;
+                    pw_panel<true, AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
+                    if (tie) sh.tie = 1;
+                    pivot_warps_bar<AW>();
+                    const bool redo = sh.tie != 0;
+                    pivot_warps_bar<AW>();
+                    if (redo) { // rare: the panel again, from shared memory, ties resolved exactly
+                        if (threadIdx.x == 0) sh.tie = 0;
+#pragma unroll
+                        for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
+                        m = m_in;
+                        bad = 0u;
+                        pw_panel<false, AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
+                    }
+#pragma unroll
+                    for (int c = 0; c < FR_NB; ++c) { // the eliminated panel: in place, and into the panel buffer
+                        Wp[c * LD] = t[c];
+                        pb.T[c][r] = t[c];
+                    }
+                    if (w == 0 && lane < FR_NB) pb.R[lane] = sh.rho[FR_NB * pnl + lane];
+                    if (threadIdx.x == 0) pb.sing = bad ? 1 : 0;
+                }
+                __syncthreads(); // the panel buffer is complete
+                if (threadIdx.x == 0) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); // generic-proxy writes -> bulk-copy reads
+#pragma unroll
+                    for (int peer = 0; peer < NQ; ++peer)
+                        if (peer != q)
+                            bulk_s2peer(mapa_u32(smem_u32(&pb), peer), &pb, (uint32_t)sizeof(CqPanelBuf<NQ>),
+                                        mapa_u32(smem_u32(&sh.tfull[buf]), peer));
+                    mbar_arrive(&sh.tfull[buf]); // the owner's own copy is already in place
+                }
+            } else if (threadIdx.x == 0) {
+                mbar_arrive_expect_tx(&sh.tfull[buf], (uint32_t)sizeof(CqPanelBuf<NQ>));
+            }
+            mbar_wait(&sh.tfull[buf], par);
+            if (pb.sing) singular = true; // cluster-uniform
+            // every CTA keeps the whole permutation and the used-row masks (any CTA may own a later panel)
+            if (q != owner && threadIdx.x < FR_NB) {
+                const int r = pb.R[threadIdx.x];
+                sh.rho[FR_NB * pnl + threadIdx.x] = r;
+                sh.rhoinv[r] = FR_NB * pnl + threadIdx.x;
+            }
+            if (q != owner && w < AW) {
+#pragma unroll
+                for (int b = 0; b < FR_NB; ++b)
+                    if (pb.R[b] == 32 * w + lane) m = 0u;
+            }
+            if (!singular) {
+                // ================= phase U: this CTA's column blocks, one warp per block =================
+                const int rk0 = pb.R[lq], rk1 = pb.R[4 + lq];
+                for (int Jb = w; Jb < 8; Jb += NWARP) {
+                    if (q == owner && Jb == lb) continue;
+                    const int cl = wc2_colmap(lg);
+                    double *a0p = &W[(8 * Jb + cl) * LD + rk0], *a1p = &W[(8 * Jb + cl) * LD + rk1];
+                    const double a0 = *a0p, a1 = *a1p;
+                    __syncwarp();
+                    *a0p = 0.0;
+                    *a1p = 0.0;
+                    __syncwarp();
+                    double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]);
+#pragma unroll 8
+                    for (int I = 0; I < n / 8; ++I) {
+                        const double z0 = pb.T[lq][8 * I + lg], z1 = pb.T[4 + lq][8 * I + lg];
+                        double2 v = cp[4 * I];
+                        dmma884(v.x, v.y, a0, z0);
+                        dmma884(v.x, v.y, a1, z1);
+                        cp[4 * I] = v;
+                    }
+                }
+            }
+            cluster_sync_all(); // updates complete everywhere; panel buffer `buf ^ 1` may be overwritten by the next owner
+            if (singular) { ++gp; break; }
+        }
+
+        double *out = Minv + (size_t)cell * n * n;
+        if (singular) {
+            if (q == 0 && threadIdx.x == 0) atomicMin(info, cell + 1);
+            for (int e = threadIdx.x; e < 64 * n / 2; e += CQ_THREADS) reinterpret_cast<double2 *>(out + (size_t)64 * q * n)[e] = make_double2(0.0, 0.0);
+            __syncthreads();
+            continue;
+        }
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]; this CTA's columns j = 64 q + jl
+        for (int jl = w; jl < 64; jl += NWARP) {
+            double *col = out + (size_t)sh.rho[64 * q + jl] * n;
+#pragma unroll
+            for (int s2 = 0; s2 < NQ; ++s2) {
+                const double2 v = *reinterpret_cast<const double2 *>(&W[jl * LD + 64 * s2 + 2 * lane]);
+                col[sh.rhoinv[64 * s2 + 2 * lane]] = v.x;
+                col[sh.rhoinv[64 * s2 + 2 * lane + 1]] = v.y;
+            }
+        }
+        __syncthreads(); // everybody is done with W before the next cell's assembly
+    }
+    cluster_sync_all(); // no CTA exits while a peer may still address its shared memory
 }
 
 __global__ void assemble_one_kernel(ProblemView P, int cell, double *__restrict__ A)
@@ -1369,6 +1571,41 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
     return 1;
 }
 
+// n = 192, 256: a cluster of NQ CTAs per cell (factor_cq_kernel). dumpA != nullptr: only assemble `dump_cell`.
+template <int NQ, bool DUMP> static int launch_factor_cq_t(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.blockDim = dim3(CQ_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = sizeof(CqShared<NQ>);
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_cq_kernel<NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)sizeof(CqShared<NQ>)));
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = NQ;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n_clusters = 1;
+    if (!DUMP) {
+        cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_cq_kernel<NQ, DUMP>, &cfg));
+        if (n_clusters < 1) n_clusters = 1;
+        if (n_clusters > ctx->J) n_clusters = ctx->J;
+    }
+    cfg.gridDim = dim3(NQ * n_clusters, 1, 1);
+    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_cq_kernel<NQ, DUMP>, P, ctx->Minv, ctx->info, dumpA, dump_cell));
+    return 1;
+}
+
+static int launch_factor_cq(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
+{
+    if (ctx->n == 192) return dumpA ? launch_factor_cq_t<3, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<3, false>(ctx, P, nullptr, 0);
+    return dumpA ? launch_factor_cq_t<4, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<4, false>(ctx, P, nullptr, 0);
+}
+
 // n = 128, one CTA per cell (factor_p128_kernel). dumpA != nullptr: only assemble `dump_cell` and write the tile there.
 static int launch_factor_p128(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
 {
@@ -1397,6 +1634,7 @@ int launch_factor(oci_ctx *ctx)
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info, 0x7f, sizeof(int), ctx->stream)); // 0x7f7f7f7f = "none"
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && n == 64) return launch_factor_wc(ctx, P, nullptr, 0);
     if (ctx->opt_factor_kernel == 1 && n == 128) return launch_factor_p128(ctx, P, nullptr, 0);
+    if (ctx->opt_factor_kernel == 1 && (n == 192 || n == 256)) return launch_factor_cq(ctx, P, nullptr, 0);
     if (ctx->opt_factor_kernel >= 1 && n % 64 == 0 && n <= 256) // 2: the 8-warp kernel also for n = 64
         return launch_factor_reg_n(ctx, P, nullptr, 0);
     const bool global_w = factor_smem_bytes(n, false) > (size_t)ctx->max_smem_optin;
@@ -1430,6 +1668,7 @@ int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor)
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && ctx->n == 64)
         return launch_factor_wc(ctx, P, A_dev_rowmajor, cell);
     if (ctx->opt_factor_kernel == 1 && ctx->n == 128) return launch_factor_p128(ctx, P, A_dev_rowmajor, cell);
+    if (ctx->opt_factor_kernel == 1 && (ctx->n == 192 || ctx->n == 256)) return launch_factor_cq(ctx, P, A_dev_rowmajor, cell);
     if (ctx->opt_factor_kernel >= 1 && ctx->n % 64 == 0 && ctx->n <= 256) return launch_factor_reg_n(ctx, P, A_dev_rowmajor, cell);
     return 0;
 }
