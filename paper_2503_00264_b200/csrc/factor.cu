@@ -483,6 +483,47 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
         : "d"(a), "d"(b));
 }
 
+// NT row tiles (8 rows each) of one column block: v[tile] += a0 z0[tile] + a1 z1[tile], the transposed rank-8 update of
+// wc2_update_blocks with the B fragments (z0, z1: the eliminated panel) read from shared memory. Software-pipelined by
+// hand: the compiler must assume that the store of a tile aliases the loads of the next one and, left alone, emits
+// load -> DMMA -> dependent DMMA -> store tile after tile (~100 cycles of exposed latency per tile). Here the loads of
+// the next four tiles are issued before the DMMAs of the current four, and the two dependent DMMAs of a tile are four
+// issue slots (~66 cycles) apart, so the warp is bound by the 16.5 cycles a DMMA occupies its sub-partition's pipe.
+// cp: the lane's double2 of tile 0 (tile stride: 4 double2 = 8 rows); zp0 / zp1: the lane's B-fragment entries of tile 0
+// (tile stride 8 doubles).
+template <int NT>
+__device__ __forceinline__ void dmma_strip(double2 *cp, const double *zp0, const double *zp1, double a0, double a1)
+{
+    static_assert(NT % 4 == 0, "tiles are processed four at a time");
+    double2 v[2][4];
+    double z0[2][4], z1[2][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        v[0][i] = cp[4 * i];
+        z0[0][i] = zp0[8 * i];
+        z1[0][i] = zp1[8 * i];
+    }
+#pragma unroll
+    for (int bt = 0; bt < NT / 4; ++bt) {
+        const int cur = bt & 1;
+        if (bt + 1 < NT / 4) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int I = 4 * (bt + 1) + i;
+                v[cur ^ 1][i] = cp[4 * I];
+                z0[cur ^ 1][i] = zp0[8 * I];
+                z1[cur ^ 1][i] = zp1[8 * I];
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dmma884(v[cur][i].x, v[cur][i].y, a0, z0[cur][i]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dmma884(v[cur][i].x, v[cur][i].y, a1, z1[cur][i]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) cp[4 * (4 * bt + i)] = v[cur][i];
+    }
+}
+
 // a1 for one warp: rows {2 lane, 2 lane + 1} of every column of A_j into the column-major shared-memory array W
 // (leading dimension ld). Same operations in the same order as a_entry(): bit-identical (asserted by
 // tests/test_gpu_parity.py::test_production_assembly_bit_exact through oci_debug_get_factor_input).
@@ -1023,12 +1064,11 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
 //     stores) separates update and panel -- while the four update warps apply the update to the other 14 blocks.
 constexpr int P128_LD = 132, P128_THREADS = 256, P128_AW = 4;
 
-struct alignas(16) P128Slot {
-    double row[FR_NB];
-    unsigned long long key; // |candidate| as an integer key (0: this warp has no unused row)
-    int lane;               // lane of the candidate; bit 8: more lanes of the warp share its high key word
+struct alignas(16) P128Slot { // five 16-byte stores per candidate: a barrier waits for the stores in flight
+    double row[FR_NB];        // the candidate's panel row as it stands; column b of step b holds 1 / candidate instead
+    unsigned long long key;   // |candidate| as an integer key (0: this warp has no unused row)
+    int lane;                 // lane of the candidate; bit 8: more lanes of the warp share its high key word
     int pad;
-    double linv, pad2;
 };
 
 struct P128Shared {
@@ -1044,8 +1084,8 @@ __device__ __forceinline__ void p128_bar_pivot() { pivot_warps_bar<P128_AW>(); }
 
 // One pivot step of a panel shared by AW pivot warps, one row per lane (row 32 w + lane). slots: [2][AW].
 template <int b, bool FAST, int AW>
-__device__ __forceinline__ void pw_pivot_step(double (&t)[FR_NB], unsigned &m, P128Slot *slots, int *rho, int *rhoinv, int w,
-                                              int lane, int col0, unsigned &bad, unsigned &tie)
+__device__ __forceinline__ void pw_pivot_step(double (&t)[FR_NB], unsigned &m, P128Slot *slots, int &myr, int w, int lane,
+                                              unsigned &bad, unsigned &tie)
 {
     constexpr unsigned FULL = 0xffffffffu;
     const unsigned h = (unsigned)__double2hiint(t[b]) & m, l = (unsigned)__double2loint(t[b]);
@@ -1062,40 +1102,60 @@ __device__ __forceinline__ void pw_pivot_step(double (&t)[FR_NB], unsigned &m, P
     P128Slot *mine = &slots[(b & 1) * AW + w];
     if (lane == src) { // this warp's candidate: key, row as it stands, 1 / candidate
 #pragma unroll
-        for (int c = 0; c < FR_NB / 2; ++c) reinterpret_cast<double2 *>(mine->row)[c] = make_double2(t[2 * c], t[2 * c + 1]);
-        mine->linv = linv;
-        mine->key = ((unsigned long long)h << 32) | l; // h == 0: no unused row here (loses, or the cell is singular)
-        mine->lane = lane | (tied ? 0x100 : 0);
+        for (int c = 0; c < FR_NB / 2; ++c)
+            reinterpret_cast<double2 *>(mine->row)[c] = make_double2(2 * c == b ? linv : t[2 * c], 2 * c + 1 == b ? linv : t[2 * c + 1]);
+        // h == 0: no unused row here (loses, or the cell is singular)
+        *reinterpret_cast<uint4 *>(&mine->key) = make_uint4(l, h, (unsigned)lane | (tied ? 0x100u : 0u), 0u);
     }
     pivot_warps_bar<AW>();
-    // the AW candidates: key and lane word of a slot in one 16-byte broadcast load
-    unsigned long long kk[AW];
-    int lw4[AW];
+    int gw, lwv;
+    if (FAST) {
+        // the AW candidates, one per lane: high key word and lane word of slot `lane` in one 16-byte load, arg-max by
+        // redux + ballot (the lowest warp = the lowest row wins). Only high words are compared here: two warps with the
+        // same maximal high word, or a winner whose warp recorded a tie of its own, mean "replay the panel exactly"
+        // (most warps tie all the time on the identical entries -dx K w / 4 of Eq. 10, far below the pivot: that is
+        // why a warp's own tie counts only when its high word is the winning one)
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (lane < AW) v = *reinterpret_cast<const uint4 *>(&slots[(b & 1) * AW + lane].key);
+        const unsigned mh2 = __reduce_max_sync(FULL, v.y);
+        const bool top = lane < AW && v.y == mh2;
+        const unsigned ball2 = __ballot_sync(FULL, top);
+        const unsigned tb = __ballot_sync(FULL, top && (v.z & 0x100u));
+        gw = (__ffs(ball2) - 1) & 31;
+        tie |= ((ball2 & (ball2 - 1u)) | tb) ? 1u : 0u;
+        lwv = __shfl_sync(FULL, (int)v.z, gw);
+        bad |= (mh2 - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot
+    } else {
+        // exact form: 64-bit keys; key and lane word of a slot in one 16-byte broadcast load
+        unsigned long long kk[AW];
+        int lw4[AW];
 #pragma unroll
-    for (int ww = 0; ww < AW; ++ww) {
-        const uint4 v = *reinterpret_cast<const uint4 *>(&slots[(b & 1) * AW + ww].key);
-        kk[ww] = ((unsigned long long)v.y << 32) | v.x;
-        lw4[ww] = (int)v.z;
+        for (int ww = 0; ww < AW; ++ww) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(&slots[(b & 1) * AW + ww].key);
+            kk[ww] = ((unsigned long long)v.y << 32) | v.x;
+            lw4[ww] = (int)v.z;
+        }
+        unsigned long long kmax = kk[0];
+        gw = 0;
+        lwv = lw4[0];
+#pragma unroll
+        for (int ww = 1; ww < AW; ++ww) // strict >: a tie goes to the lower warp, i.e. the lower row
+            if (kk[ww] > kmax) { kmax = kk[ww]; gw = ww; lwv = lw4[ww]; }
+        bad |= ((unsigned)(kmax >> 32) - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot
     }
-    unsigned long long kmax = kk[0];
-    int gw = 0, lwv = lw4[0];
-#pragma unroll
-    for (int ww = 1; ww < AW; ++ww) // strict >: a tie goes to the lower warp, i.e. the lower row
-        if (kk[ww] > kmax) { kmax = kk[ww]; gw = ww; lwv = lw4[ww]; }
-    if (FAST) { // an unresolved tie matters only where it could have hidden the true maximum: in a warp whose published
-                // high word equals the winning one (most warps tie on the identical entries -dx K w / 4 of Eq. 10, far
-                // below the pivot)
-#pragma unroll
-        for (int ww = 0; ww < AW; ++ww)
-            if ((lw4[ww] & 0x100) && (unsigned)(kk[ww] >> 32) == (unsigned)(kmax >> 32)) tie |= 1u;
-    }
-    bad |= ((unsigned)(kmax >> 32) - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot
     const P128Slot *win = &slots[(b & 1) * AW + gw];
-    const double ls = win->linv;
-    const int lw = lwv & 31;
-    double sp[FR_NB];
+    double sp[FR_NB]; // pivot row / pivot; column b holds 1 / pivot
 #pragma unroll
-    for (int c = 0; c < FR_NB; ++c) sp[c] = (c == b) ? ls : win->row[c] * ls;
+    for (int c = 0; c < FR_NB / 2; ++c) {
+        const double2 v = reinterpret_cast<const double2 *>(win->row)[c];
+        sp[2 * c] = v.x;
+        sp[2 * c + 1] = v.y;
+    }
+    const double ls = sp[b];
+    const int lw = lwv & 31;
+#pragma unroll
+    for (int c = 0; c < FR_NB; ++c)
+        if (c != b) sp[c] *= ls;
     const bool is_p = gw == w && lane == lw;
     const double f = t[b];
 #pragma unroll
@@ -1104,25 +1164,26 @@ __device__ __forceinline__ void pw_pivot_step(double (&t)[FR_NB], unsigned &m, P
         t[c] = is_p ? sp[c] : u;
     }
     m = is_p ? 0u : m;
-    if (w == 0 && lane == b) {
-        const int r = 32 * gw + lw;
-        rho[col0 + b] = r;
-        rhoinv[r] = col0 + b;
-    }
+    if (lane == b) myr = 32 * gw + lw; // lane b keeps pivot row b: stored once per panel (pw_panel)
 }
 
 template <bool FAST, int AW>
 __device__ __forceinline__ void pw_panel(double (&t)[FR_NB], unsigned &m, P128Slot *slots, int *rho, int *rhoinv, int w, int lane,
                                          int col0, unsigned &bad, unsigned &tie)
 {
-    pw_pivot_step<0, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<1, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<2, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<3, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<4, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<5, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<6, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
-    pw_pivot_step<7, FAST, AW>(t, m, slots, rho, rhoinv, w, lane, col0, bad, tie);
+    int myr = 0;
+    pw_pivot_step<0, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<1, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<2, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<3, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<4, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<5, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<6, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    pw_pivot_step<7, FAST, AW>(t, m, slots, myr, w, lane, bad, tie);
+    if (w == 0 && lane < FR_NB) { // the panel's pivot rows (stores kept out of the steps: the step barrier waits for them)
+        rho[col0 + lane] = myr;
+        rhoinv[myr] = col0 + lane;
+    }
 }
 
 // one whole column block by one warp (see wc2_update_blocks): pivot rows read, zeroed, 16 row tiles updated
@@ -1271,8 +1332,14 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
 // singular flag then travel ONCE to every other CTA of the cluster: the owner writes them to its own panel buffer and
 // one thread issues a bulk asynchronous copy (cp.async.bulk shared::cta -> shared::cluster, completion on the
 // receiver's mbarrier) per peer; every CTA then applies the rank-8 update to its own eight column blocks (transposed
-// m8n8k4 DMMAs, pivot rows zeroed, one warp per block) from its local copy. One cluster barrier per panel orders the
-// re-use of the two panel buffers and the hand-over of the pivot role from CTA to CTA.
+// m8n8k4 DMMAs, one warp per block) from its local copy.
+// Look-ahead: in the CTA that owns panel p + 1 the pivot warps update only that panel's block (warp w the 32 rows it then
+// loads) and go straight on to eliminate it, while the remaining warps apply update p to the CTA's other blocks; the
+// other CTAs update all their blocks. The critical path of a cell is its n pivot steps plus n / 8 one-block updates and
+// stays inside one SM except at the eight-panel hand-over from CTA to CTA. No cluster barrier inside a cell: the two
+// panel buffers are recycled through mbarriers -- `tfull` (the copy of panel p has landed here) and `tempty` (every peer
+// has finished reading panel p: each CTA arrives remotely on all its peers' barriers after the CTA barrier that follows
+// its update p, so the phase of every barrier is a function of the panel count alone).
 constexpr int CQ_THREADS = 384; // 12 warps: the first n / 32 are pivot warps when the CTA owns the panel
 
 template <int NQ> struct CqPanelBuf {
@@ -1286,6 +1353,7 @@ template <int NQ> struct CqShared {
     CqPanelBuf<NQ> pb[2];             // [panel parity]
     P128Slot slot[2][2 * NQ];         // [step parity][pivot warp]
     uint64_t tfull[2];                // panel buffer `parity` holds panel p
+    uint64_t tempty[2];               // every peer has finished reading panel buffer `parity`
     int rho[64 * NQ], rhoinv[64 * NQ];
     int tie;
 };
@@ -1302,6 +1370,10 @@ __device__ __forceinline__ void bulk_s2peer(uint32_t dst_cluster, const void *sr
                  "r"(smem_u32(src_smem)), "r"(bytes), "r"(bar_cluster)
                  : "memory");
 }
+__device__ __forceinline__ void mbar_arrive_peer(uint32_t bar_cluster)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+}
 __device__ __forceinline__ void cluster_sync_all()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -1313,11 +1385,27 @@ __device__ __forceinline__ uint32_t cluster_ctarank()
     return r;
 }
 
+// one whole column block of a CTA's 64 columns by one warp: pivot rows read, zeroed, n / 8 row tiles updated
+template <int NQ>
+__device__ __forceinline__ void cq_update_block(double *W, const CqPanelBuf<NQ> &pb, int Jb, int rk0, int rk1, int lq, int lg)
+{
+    constexpr int n = 64 * NQ, LD = n + 4;
+    const int cl = wc2_colmap(lg);
+    double *a0p = &W[(8 * Jb + cl) * LD + rk0], *a1p = &W[(8 * Jb + cl) * LD + rk1];
+    const double a0 = *a0p, a1 = *a1p;
+    __syncwarp();
+    *a0p = 0.0;
+    *a1p = 0.0;
+    __syncwarp();
+    dmma_strip<n / 8>(reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]), &pb.T[lq][lg], &pb.T[4 + lq][lg], a0, a1);
+}
+
 template <int NQ, bool DUMP>
 __global__ void __launch_bounds__(CQ_THREADS, 1)
 factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__restrict__ dumpA, int dump_cell)
 {
-    constexpr int n = 64 * NQ, LD = n + 4, NPANEL = n / FR_NB, AW = 2 * NQ, NWARP = CQ_THREADS / 32;
+    constexpr int n = 64 * NQ, LD = n + 4, NPANEL = n / FR_NB, AW = 2 * NQ, NWARP = CQ_THREADS / 32, UW = NWARP - AW;
+    constexpr int SENDER = CQ_THREADS - 32; // lane 0 of the last warp: never on the pivot chain, least update work
     extern __shared__ __align__(16) unsigned char cq_smem[];
     CqShared<NQ> &sh = *reinterpret_cast<CqShared<NQ> *>(cq_smem);
     double *W = sh.W;
@@ -1328,11 +1416,20 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
     if (threadIdx.x == 0) {
         mbar_init(&sh.tfull[0], 1);
         mbar_init(&sh.tfull[1], 1);
+        mbar_init(&sh.tempty[0], NQ - 1);
+        mbar_init(&sh.tempty[1], NQ - 1);
         fence_mbar_init();
         sh.tie = 0;
     }
-    cluster_sync_all(); // barriers initialised everywhere before any peer copies into this CTA
-    unsigned gp = 0;    // panels processed so far by this cluster (selects buffer and barrier parity)
+    cluster_sync_all(); // barriers initialised everywhere before any peer copies into this CTA or arrives here
+    unsigned gp = 0;    // panels processed so far by this cluster (selects buffer and barrier parities)
+
+    // "this CTA has finished reading panel buffer b": one remote arrival on every peer's tempty[b]
+    auto release_panel_buffer = [&](int b) {
+#pragma unroll
+        for (int peer = 0; peer < NQ; ++peer)
+            if (peer != q) mbar_arrive_peer(mapa_u32(smem_u32(&sh.tempty[b]), peer));
+    };
 
     for (int cell = DUMP ? dump_cell : cluster_id; cell < P.J; cell += n_clusters) {
         // ---- a1: this CTA's 64 columns (16 column blocks of 4) x n rows
@@ -1352,40 +1449,46 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
         for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
             const int owner = pnl >> 3, lb = pnl & 7, buf = gp & 1;
             const uint32_t par = (gp >> 1) & 1;
+            const bool own = q == owner, own_next = pnl + 1 < NPANEL && q == ((pnl + 1) >> 3);
             CqPanelBuf<NQ> &pb = sh.pb[buf];
-            if (q == owner) {
-                if (w < AW) {
-                    // ================= phase P: the owner's pivot warps eliminate the n x 8 panel, one row per lane =========
-                    const int r = 32 * w + lane;
-                    double *Wp = &W[(FR_NB * lb) * LD + r];
-                    double t[FR_NB];
+            if (own && w < AW) {
+                // ================= phase P: the owner's pivot warps eliminate the n x 8 panel, one row per lane =========
+                // (its block is up to date: updates < pnl - 1 by the update warps before the last CTA barrier, update
+                // pnl - 1 by this very warp, rows 32 w .. 32 w + 31, in the look-ahead below)
+                const int r = 32 * w + lane;
+                double *Wp = &W[(FR_NB * lb) * LD + r];
+                double t[FR_NB];
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
+                unsigned bad = 0u, tie = 0u;
+                const unsigned m_in = m;
+                pw_panel<true, AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
+                if (tie) sh.tie = 1;
+                pivot_warps_bar<AW>();
+                const bool redo = sh.tie != 0;
+                pivot_warps_bar<AW>();
+                if (redo) { // rare: the panel again, from shared memory, ties resolved exactly
+                    if (threadIdx.x == 0) sh.tie = 0;
 #pragma unroll
                     for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
-                    unsigned bad = 0u, tie = 0u;
-                    const unsigned m_in = m;
-                    pw_panel<true, AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
-                    if (tie) sh.tie = 1;
-                    pivot_warps_bar<AW>();
-                    const bool redo = sh.tie != 0;
-                    pivot_warps_bar<AW>();
-                    if (redo) { // rare: the panel again, from shared memory, ties resolved exactly
-                        if (threadIdx.x == 0) sh.tie = 0;
-#pragma unroll
-                        for (int c = 0; c < FR_NB; ++c) t[c] = Wp[c * LD];
-                        m = m_in;
-                        bad = 0u;
-                        pw_panel<false, AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
-                    }
-#pragma unroll
-                    for (int c = 0; c < FR_NB; ++c) { // the eliminated panel: in place, and into the panel buffer
-                        Wp[c * LD] = t[c];
-                        pb.T[c][r] = t[c];
-                    }
-                    if (w == 0 && lane < FR_NB) pb.R[lane] = sh.rho[FR_NB * pnl + lane];
-                    if (threadIdx.x == 0) pb.sing = bad ? 1 : 0;
+                    m = m_in;
+                    bad = 0u;
+                    pw_panel<false, AW>(t, m, &sh.slot[0][0], sh.rho, sh.rhoinv, w, lane, FR_NB * pnl, bad, tie);
                 }
-                __syncthreads(); // the panel buffer is complete
-                if (threadIdx.x == 0) {
+                // the panel buffer is free once every peer has finished reading the panel before last (which also means
+                // that the bulk copies out of it have completed)
+                if (gp >= 2) mbar_wait(&sh.tempty[buf], ((gp >> 1) - 1) & 1);
+#pragma unroll
+                for (int c = 0; c < FR_NB; ++c) { // the eliminated panel: in place, and into the panel buffer
+                    Wp[c * LD] = t[c];
+                    pb.T[c][r] = t[c];
+                }
+                if (w == 0 && lane < FR_NB) pb.R[lane] = sh.rho[FR_NB * pnl + lane];
+                if (threadIdx.x == 0) pb.sing = bad ? 1 : 0;
+            }
+            __syncthreads(); // barrier p: update p - 1 is complete in this CTA; in the owner, the panel buffer is complete
+            if (threadIdx.x == SENDER) {
+                if (own) {
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); // generic-proxy writes -> bulk-copy reads
 #pragma unroll
                     for (int peer = 0; peer < NQ; ++peer)
@@ -1393,49 +1496,94 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
                             bulk_s2peer(mapa_u32(smem_u32(&pb), peer), &pb, (uint32_t)sizeof(CqPanelBuf<NQ>),
                                         mapa_u32(smem_u32(&sh.tfull[buf]), peer));
                     mbar_arrive(&sh.tfull[buf]); // the owner's own copy is already in place
+                } else {
+                    mbar_arrive_expect_tx(&sh.tfull[buf], (uint32_t)sizeof(CqPanelBuf<NQ>));
                 }
-            } else if (threadIdx.x == 0) {
-                mbar_arrive_expect_tx(&sh.tfull[buf], (uint32_t)sizeof(CqPanelBuf<NQ>));
+                if (pnl > 0) release_panel_buffer(buf ^ 1); // nobody here reads the previous panel any more (a cell's last
+                                                             // panel is released after the loop)
             }
-            mbar_wait(&sh.tfull[buf], par);
-            if (pb.sing) singular = true; // cluster-uniform
+            if (!own) mbar_wait(&sh.tfull[buf], par);
+            if (pb.sing) { singular = true; ++gp; break; } // cluster-uniform
             // every CTA keeps the whole permutation and the used-row masks (any CTA may own a later panel)
-            if (q != owner && threadIdx.x < FR_NB) {
+            if (!own && threadIdx.x < FR_NB) {
                 const int r = pb.R[threadIdx.x];
                 sh.rho[FR_NB * pnl + threadIdx.x] = r;
                 sh.rhoinv[r] = FR_NB * pnl + threadIdx.x;
             }
-            if (q != owner && w < AW) {
+            if (!own && w < AW) {
 #pragma unroll
                 for (int b = 0; b < FR_NB; ++b)
                     if (pb.R[b] == 32 * w + lane) m = 0u;
             }
-            if (!singular) {
-                // ================= phase U: this CTA's column blocks, one warp per block =================
-                const int rk0 = pb.R[lq], rk1 = pb.R[4 + lq];
-                for (int Jb = w; Jb < 8; Jb += NWARP) {
-                    if (q == owner && Jb == lb) continue;
-                    const int cl = wc2_colmap(lg);
-                    double *a0p = &W[(8 * Jb + cl) * LD + rk0], *a1p = &W[(8 * Jb + cl) * LD + rk1];
-                    const double a0 = *a0p, a1 = *a1p;
-                    __syncwarp();
-                    *a0p = 0.0;
-                    *a1p = 0.0;
-                    __syncwarp();
-                    double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]);
-#pragma unroll 8
-                    for (int I = 0; I < n / 8; ++I) {
-                        const double z0 = pb.T[lq][8 * I + lg], z1 = pb.T[4 + lq][8 * I + lg];
-                        double2 v = cp[4 * I];
-                        dmma884(v.x, v.y, a0, z0);
-                        dmma884(v.x, v.y, a1, z1);
-                        cp[4 * I] = v;
+            // ================= phase U: this CTA's column blocks =================
+            const int rk0 = pb.R[lq], rk1 = pb.R[4 + lq];
+            const int nb = (pnl + 1) & 7; // block of the next panel (when this CTA owns it)
+            if (own_next && w < AW) {
+                // look-ahead: the next panel's block, pivot warp w its own 32 rows (row tiles 4 w .. 4 w + 3). Every pivot
+                // warp reads the pivot-row entries of the block, one barrier over the pivot warps, then each warp zeroes
+                // the pivot rows that lie in its own 32 rows (see wc2_update_blocks) and accumulates.
+                const int cl = wc2_colmap(lg);
+                double *a0p = &W[(8 * nb + cl) * LD + rk0], *a1p = &W[(8 * nb + cl) * LD + rk1];
+                const double a0 = *a0p, a1 = *a1p;
+                pivot_warps_bar<AW>(); // every pivot warp has read the pivot rows of the block
+                if ((rk0 >> 5) == w) *a0p = 0.0;
+                if ((rk1 >> 5) == w) *a1p = 0.0;
+                __syncwarp();
+                dmma_strip<4>(reinterpret_cast<double2 *>(&W[(8 * nb + cl) * LD + 2 * lq + 32 * w]), &pb.T[lq][32 * w + lg],
+                              &pb.T[4 + lq][32 * w + lg], a0, a1);
+                __syncwarp();
+            } else if (own_next) {
+                // the update warps while the pivot warps are busy with the next panel: this CTA's other six or seven
+                // blocks as half-blocks (n / 2 rows), shared out round-robin (the last warp, which is also the sender,
+                // gets the fewest). The pivot-row entries of a block are read by everybody before anybody stores (named
+                // barrier over the update warps); each warp then zeroes the pivot rows that lie in its own half.
+                const int wi = w - AW;
+                const int s1 = own ? (lb < nb ? lb : nb) : nb, s2 = own ? (lb < nb ? nb : lb) : 99; // skipped blocks, sorted
+                const int nitems = 2 * (own ? 6 : 7);
+                constexpr int MAXIT = (14 + UW - 1) / UW;
+                const int cl = wc2_colmap(lg);
+                double a0[MAXIT], a1[MAXIT];
+                int jb[MAXIT];
+#pragma unroll
+                for (int sl = 0; sl < MAXIT; ++sl) {
+                    const int it = wi + sl * UW;
+                    int Jb = it >> 1;
+                    if (Jb >= s1) ++Jb;
+                    if (Jb >= s2) ++Jb;
+                    jb[sl] = Jb;
+                    if (it < nitems) {
+                        a0[sl] = W[(8 * Jb + cl) * LD + rk0];
+                        a1[sl] = W[(8 * Jb + cl) * LD + rk1];
+                    }
+                }
+                asm volatile("bar.sync 2, %0;" ::"n"(32 * UW) : "memory");
+#pragma unroll
+                for (int sl = 0; sl < MAXIT; ++sl) {
+                    const int it = wi + sl * UW;
+                    if (it < nitems) {
+                        const int r0 = (it & 1) * (n / 2); // first row of the half
+                        double *col = &W[(8 * jb[sl] + cl) * LD];
+                        if ((unsigned)(rk0 - r0) < (unsigned)(n / 2)) col[rk0] = 0.0;
+                        if ((unsigned)(rk1 - r0) < (unsigned)(n / 2)) col[rk1] = 0.0;
+                        __syncwarp();
+                        dmma_strip<n / 16>(reinterpret_cast<double2 *>(col + 2 * lq + r0), &pb.T[lq][r0 + lg], &pb.T[4 + lq][r0 + lg],
+                                           a0[sl], a1[sl]);
+                    }
+                }
+            } else {
+                // nobody here is on the pivot chain: whole blocks, one per warp, on the first eight warps
+                if (w < 8) {
+                    int k = 0;
+                    for (int Jb = 0; Jb < 8; ++Jb) {
+                        if (own && Jb == lb) continue;
+                        if (k == w) cq_update_block<NQ>(W, pb, Jb, rk0, rk1, lq, lg);
+                        k = (k + 1 == 8) ? 0 : k + 1;
                     }
                 }
             }
-            cluster_sync_all(); // updates complete everywhere; panel buffer `buf ^ 1` may be overwritten by the next owner
-            if (singular) { ++gp; break; }
         }
+        __syncthreads(); // the last update is complete (or the cell was found singular)
+        if (threadIdx.x == SENDER) release_panel_buffer((gp - 1) & 1);
 
         double *out = Minv + (size_t)cell * n * n;
         if (singular) {
