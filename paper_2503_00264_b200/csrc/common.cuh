@@ -135,6 +135,7 @@ struct IterParams {
     int stages;   // matrix ring depth
     int chunk_doubles;
     int color, ncolors;   // structured path: cells j = ncolors * i + color (ncolors = 1: all cells)
+    int reverse;  // warp-per-cell kernel: every CTA walks its range of cells from the top down (see iterate.cu)
 };
 
 // opt-in dynamic shared memory for `fn`, once per (context, kernel, size)

@@ -287,6 +287,14 @@ __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const I
     // balanced contiguous split of the cells over the CTAs
     const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
     const int cell1 = (int)(((long long)J * (blockIdx.x + 1)) / gridDim.x);
+    // Successive iterations walk the range in opposite directions (P.reverse = parity of the history slot): a Jacobi
+    // iteration does not care about the order of its cells, and the inverses, c and Psi a CTA touched last in iteration l
+    // are then the first it asks for in iteration l + 1, while they are still in the L2 (126 MB against 2.1 GB of
+    // inverses on config 5: a per cent of the stream, for nothing). Slot 0 walks down: oci_factor writes the inverses
+    // in ascending order. Walking down, the groups of WPC_WARPS cells are counted from the top, so that the ragged
+    // group is the LAST one in either direction (a warp without a cell skips its ring slots, which is only
+    // consistent with the producer's parities when nothing follows).
+    const int ngroups = (cell1 - cell0 + WPC_WARPS - 1) / WPC_WARPS;
 
     if (warp == WPC_WARPS) {
         // ===================== producer ==================================================================
@@ -294,8 +302,9 @@ __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const I
             int vs = 0;
             uint32_t vph = 0;
             unsigned it = 0; // chunk round: every warp with a cell gets one chunk per round
-            for (int gb = cell0; gb < cell1; gb += WPC_WARPS) {
-                const int nv = min(WPC_WARPS, cell1 - gb);
+            for (int gi = 0; gi < ngroups; ++gi) {
+                const int gb = P.reverse ? max(cell0, cell1 - WPC_WARPS * (gi + 1)) : cell0 + WPC_WARPS * gi;
+                const int nv = P.reverse ? cell1 - WPC_WARPS * gi - gb : min(WPC_WARPS, cell1 - gb);
                 mbar_wait(&vec_empty[vs], vph ^ 1);
                 {
                     double *cs = vec + (size_t)vs * (vec_c + vec_nb);
@@ -329,8 +338,9 @@ __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const I
     uint32_t vph = 0;
     unsigned it = 0;
     double rmax = 0.0, l2 = 0.0;
-    for (int gb = cell0; gb < cell1; gb += WPC_WARPS) {
-        const int nv = min(WPC_WARPS, cell1 - gb);
+    for (int gi = 0; gi < ngroups; ++gi) {
+        const int gb = P.reverse ? max(cell0, cell1 - WPC_WARPS * (gi + 1)) : cell0 + WPC_WARPS * gi;
+        const int nv = P.reverse ? cell1 - WPC_WARPS * gi - gb : min(WPC_WARPS, cell1 - gb);
         double *cs = vec + (size_t)vs * (vec_c + vec_nb);
         const double *nb = cs + vec_c;
         mbar_wait(&vec_full[vs], vph);
@@ -692,7 +702,8 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
     P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
     P.resid_inf = ctx->resid_inf + hist_slot;
     P.resid_l2 = ctx->resid_l2 + hist_slot;
-    P.color = 0; P.ncolors = 1;
+    P.color = 0; P.ncolors = 1; P.reverse = 0;
+    P.reverse = (hist_slot & 1) == 0;
     if (ctx->opt_ordering == 1 && ctx->opt_solve_mode != 1) return OCI_E_UNSUPPORTED; // red-black: structured path only
     const bool wpc_ok = ctx->n == 64 || ctx->n == 128 || ctx->n == 256;
     if (ctx->opt_solve_mode == 1) {
@@ -818,7 +829,7 @@ int launch_dense_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_
     P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
     P.resid_inf = ctx->resid_inf + slot0; P.resid_l2 = ctx->resid_l2 + slot0;
     P.cpb = 1; P.S = 1; P.cw = n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
-    P.color = 0; P.ncolors = 1;
+    P.color = 0; P.ncolors = 1; P.reverse = 0;
     DenseMulti M;
     M.n_iters = k; M.slot0 = slot0; M.check_between = check_between ? 1 : 0; M.rule = ctx->stop_rule; M.tol = ctx->stop_tol;
     M.cpc = cpc;

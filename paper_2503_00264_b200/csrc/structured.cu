@@ -488,13 +488,19 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
 
     const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
     const int cell1 = (int)(((long long)J * (blockIdx.x + 1)) / gridDim.x);
+    // successive iterations walk the range in opposite directions (P.reverse, see oci_iterate_wpc_kernel): what a CTA
+    // touched last is what it asks for first next time, while it is still in the L2 -- here an iteration's whole stream
+    // (164 MB on config 5) is of the order of the L2
+    const int nbatch = (cell1 - cell0 + CPB - 1) / CPB;
+    auto batch_first = [&](int bi) { return cell0 + CPB * (P.reverse ? nbatch - 1 - bi : bi); };
 
     if (warp == STP_CONSUMERS / 32) {
         // ===================== producer =====================================================================
         if (lane == 0) {
             int st = 0;
             uint32_t ph = 0;
-            for (int gb = cell0; gb < cell1; gb += CPB) {
+            for (int bi = 0; bi < nbatch; ++bi) {
+                const int gb = batch_first(bi);
                 const int nb = min(CPB, cell1 - gb);
                 mbar_wait(&empty[st], ph ^ 1);
                 double *base = ring + (size_t)st * lay.doubles;
@@ -551,10 +557,11 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
             phi_old_n = P.phi[(size_t)j2 * G4 + r2];
         }
     };
-    load_role2(cell0, min(CPB, cell1 - cell0));
+    if (nbatch > 0) load_role2(batch_first(0), min(CPB, cell1 - batch_first(0)));
     int st = 0;
     uint32_t ph = 0;
-    for (int gb = cell0; gb < cell1; gb += CPB) {
+    for (int bi = 0; bi < nbatch; ++bi) {
+        const int gb = batch_first(bi);
         const int nb = min(CPB, cell1 - gb);
         const double *base = ring + (size_t)st * lay.doubles;
         const int j = gb + a;
@@ -564,7 +571,7 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
         double Kr[GC > 0 ? GC : 1], dxq = dxq_n, phi_old = phi_old_n;
 #pragma unroll
         for (int gc = 0; gc < (GC > 0 ? GC : 1); ++gc) Kr[gc] = Kr_n[gc];
-        load_role2(gb + CPB, min(CPB, cell1 - gb - CPB));
+        if (bi + 1 < nbatch) load_role2(batch_first(bi + 1), min(CPB, cell1 - batch_first(bi + 1)));
         mbar_wait(&full[st], ph);
         double z[4];
         // the two stored rows of this thread's block inverse: in registers, except for G = 8, whose instantiation has
@@ -937,7 +944,7 @@ int launch_st_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_bet
     P.inc_left = ctx->inc_left; P.inc_right = ctx->inc_right;
     P.resid_inf = ctx->resid_inf + slot0; P.resid_l2 = ctx->resid_l2 + slot0;
     P.cpb = 1; P.S = 1; P.cw = ctx->n; P.nch = 1; P.n_items = ctx->J; P.stages = 0; P.chunk_doubles = 0;
-    P.color = 0; P.ncolors = 1;
+    P.color = 0; P.ncolors = 1; P.reverse = 0;
     StParams S;
     S.LinvT = ctx->st_LinvT; S.Cinv = ctx->st_Cinv; S.dx = ctx->dx; S.transfer = ctx->transfer;
     StMulti M;
