@@ -192,6 +192,26 @@ int launch_dense_multi(oci_ctx *ctx, int slot0, int k, bool want_l2, bool check_
 int launch_si_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_prev);
 
 #ifdef __CUDACC__
+// Launch with programmatic stream serialisation: the kernel may be scheduled while its predecessor on the stream is
+// still draining, which hides the launch latency and the tail of the predecessor behind this kernel's prologue
+// (see pdl_wait below).
+template <class... KArgs, class... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // Device helpers
 // ------------------------------------------------------------------------------------------------------------
@@ -238,6 +258,14 @@ __device__ __forceinline__ double warp_sum(double v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+
+// ---- programmatic dependent launch (the per-iteration kernels of one step follow each other on one stream) ----
+// pdl_launch_dependents(): the next kernel of the stream may start launching (its CTAs take the SMs as ours leave);
+// pdl_wait(): block until the previous kernel has completed and its writes are visible. A kernel launched with
+// launch_pdl() must call pdl_wait() before it reads or writes anything the previous kernel touches. Both are no-ops in
+// a kernel launched the ordinary way.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ---- mbarrier / bulk-copy PTX wrappers ---------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)

@@ -252,8 +252,7 @@ constexpr int WPC_MAX_STAGES = 16;                // WPC_WARPS x stages per warp
 template <int RPL, bool WANT_L2>
 __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const IterParams P)
 {
-    if (stop_reached(P.stop)) return;
-    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
+    pdl_launch_dependents(); // (see launch_pdl: everything up to pdl_wait() below touches constant inputs only)
     constexpr int n = 32 * RPL;
     constexpr int CW = WPC_CHUNK / n;   // columns per chunk
     constexpr int NCH = n / CW;         // chunks per cell
@@ -283,6 +282,9 @@ __global__ void __launch_bounds__(WPC_THREADS, 1) oci_iterate_wpc_kernel(const I
     }
     for (int i = tid; i < N; i += WPC_THREADS) { mu_s[i] = P.mu[i]; w_s[i] = P.w[i]; }
     __syncthreads();
+    pdl_wait(); // the previous iteration (or whatever precedes on the stream) is complete from here on
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
 
     // balanced contiguous split of the cells over the CTAs
     const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
@@ -727,7 +729,8 @@ int launch_oci_iteration(oci_ctx *ctx, int hist_slot, bool want_l2, bool check_p
     do {                                                                                                           \
         OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_WPC + (RPL_ == 2 ? 0 : (RPL_ == 4 ? 2 : 4)) + (L2_ ? 1 : 0),         \
                                      (const void *)oci_iterate_wpc_kernel<RPL_, L2_>, smem));                      \
-        oci_iterate_wpc_kernel<RPL_, L2_><<<grid, WPC_THREADS, smem, ctx->stream>>>(P);                             \
+        OCI_CUDA_TRY(ctx, launch_pdl(oci_iterate_wpc_kernel<RPL_, L2_>, dim3(grid), dim3(WPC_THREADS), smem,        \
+                                     ctx->stream, P));                                                            \
     } while (0)
         if (n == 64) { if (want_l2) OCI_WPC_LAUNCH(2, true); else OCI_WPC_LAUNCH(2, false); }
         else if (n == 128) { if (want_l2) OCI_WPC_LAUNCH(4, true); else OCI_WPC_LAUNCH(4, false); }

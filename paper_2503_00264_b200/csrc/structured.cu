@@ -451,8 +451,7 @@ template <bool WANT_L2, int GC, int CT>
 __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_kernel(const IterParams P, const StParams S, int stages,
                                                                                      int warp_local)
 {
-    if (stop_reached(P.stop)) return;
-    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
+    pdl_launch_dependents(); // (see launch_pdl: everything up to pdl_wait() below touches constant inputs only)
     extern __shared__ __align__(128) unsigned char stp_smem[];
     const int N = P.N, G = GC > 0 ? GC : P.G, J = P.J, n = P.n, GN = G * N, G4 = 4 * G;
     constexpr int STP_CONSUMERS = CT, STP_THREADS = CT + 32;
@@ -485,6 +484,9 @@ __global__ void __launch_bounds__(CT + 32, CT == 256 ? 2 : 4) st_iterate_pipe_ke
         incr_s[i] = P.bc_right == OCI_BC_PRESCRIBED ? P.inc_right[i] : 0.0;
     }
     __syncthreads();
+    pdl_wait(); // the previous iteration (or whatever precedes on the stream) is complete from here on
+    if (stop_reached(P.stop)) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.stop.executed = P.stop.slot + 1;
 
     const int cell0 = (int)(((long long)J * blockIdx.x) / gridDim.x);
     const int cell1 = (int)(((long long)J * (blockIdx.x + 1)) / gridDim.x);
@@ -867,7 +869,8 @@ int launch_st_iteration(oci_ctx *ctx, const IterParams &P, bool want_l2)
         OCI_CUDA_TRY(ctx, grant_smem(ctx, SLOT_STP + (((GC_ == 0 ? 0 : (GC_ == 1 ? 1 : (GC_ == 2 ? 2 : (GC_ == 4 ? 3 : 4)))) * 2 + \
                                                       (CT_ == 128 ? 0 : 1)) * 2 + (L2_ ? 1 : 0)),                  \
                                      (const void *)st_iterate_pipe_kernel<L2_, GC_, CT_>, smem));                  \
-        st_iterate_pipe_kernel<L2_, GC_, CT_><<<grid, CT_ + 32, smem, ctx->stream>>>(P, S, stages, warp_local);    \
+        OCI_CUDA_TRY(ctx, launch_pdl(st_iterate_pipe_kernel<L2_, GC_, CT_>, dim3(grid), dim3(CT_ + 32), smem,      \
+                                     ctx->stream, P, S, stages, warp_local));                                    \
     } while (0)
 #define OCI_STP_G(GC_)                                                                                             \
     do {                                                                                                           \
