@@ -1069,9 +1069,11 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
 // look-ahead, optimistic branch-free panel with an exact replay on a tie of high key words. What differs:
 //   * FOUR pivot warps, one row per lane (a single warp with four rows per lane would issue ~200 instructions per
 //     pivot step in order). Per step each warp finds its own first maximal |entry| (redux + ballot), its winner
-//     publishes {64-bit key, lane, row as it stands, 1 / candidate} in a slot, one named barrier over the 128 pivot
-//     threads, every lane picks the maximal key (strict >: a tie goes to the lower warp = the lower row) and
-//     eliminates its row. Two slot sets alternate, so one barrier per step.
+//     publishes {64-bit key, lane, row as it stands with 1 / candidate in the step's column} in a slot (five 16-byte
+//     stores: the barrier that follows waits for the stores in flight), one named barrier over the 128 pivot
+//     threads, lane ww reads warp ww's key and the arg-max over the warps is a second redux + ballot (the lowest warp
+//     = the lowest row wins; the exact replay compares the 64-bit keys one after the other), and every lane eliminates
+//     its row. Two slot sets alternate, so one barrier per step; the pivot rows of a panel are stored once per panel.
 //   * Look-ahead: the pivot warps update the next panel's block -- warp w the row tiles 4 w .. 4 w + 3, which are the
 //     rows it then loads for the next panel, so nothing but one pivot-warp barrier (pivot rows read before anybody
 //     stores) separates update and panel -- while the four update warps apply the update to the other 14 blocks.
