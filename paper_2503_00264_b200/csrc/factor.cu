@@ -841,8 +841,7 @@ struct WcPanel {
 // If a panel recorded a tie it is reloaded and eliminated again with FAST = false, which resolves ties exactly (low key
 // words, then the lowest row: the first maximal |entry|, as LAPACK's idamax). Same arithmetic in both forms.
 template <int b, bool FAST>
-__device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, int *rho, int *rhoinv, int col0, int lane,
-                                               unsigned &bad, unsigned &tie)
+__device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, int &myr, int lane, unsigned &bad, unsigned &tie)
 {
     constexpr unsigned FULL = 0xffffffffu;
     // |entry| of the unused rows as integer keys (non-negative doubles order like their bit patterns); the low words
@@ -920,25 +919,26 @@ __device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, in
             if (!(FAST && c == b + 1)) R.t1[c] = sp[c];
         R.m1 = 0u;
     }
-    if (lane == b) {
-        const int r = 2 * src + esrc;
-        rho[col0 + b] = r;
-        rhoinv[r] = col0 + b;
-    }
+    if (lane == b) myr = 2 * src + esrc; // lane b keeps pivot row b: stored once per panel (wc2_panel)
 }
 
 template <bool FAST>
 __device__ __forceinline__ void wc2_panel(WcPanel &R, double *prow, int *rho, int *rhoinv, int col0, int lane, unsigned &bad,
                                           unsigned &tie)
 {
-    wc2_pivot_step<0, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<1, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<2, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<3, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<4, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<5, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<6, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
-    wc2_pivot_step<7, FAST>(R, prow, rho, rhoinv, col0, lane, bad, tie);
+    int myr = 0;
+    wc2_pivot_step<0, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<1, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<2, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<3, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<4, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<5, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<6, FAST>(R, prow, myr, lane, bad, tie);
+    wc2_pivot_step<7, FAST>(R, prow, myr, lane, bad, tie);
+    if (lane < FR_NB) { // the panel's pivot rows, once per panel
+        rho[col0 + lane] = myr;
+        rhoinv[myr] = col0 + lane;
+    }
 }
 
 template <bool DUMP>
