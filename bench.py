@@ -625,7 +625,8 @@ def run_factor_ab(args):
     p = W.config5(dt=1e-3)
     n, J = p.n, p.J
     rows = []
-    for name, opts in (("factor_wc2_kernel: 2 warps/cell, look-ahead, DMMA [production]", {}),
+    for name, opts in (("factor_wc2_kernel: 2 warps/cell, look-ahead, DMMA, panels paired [production]", {}),
+                       ("factor_wc2_kernel: the same, one rank-8 pass per panel", {"factor_update": 1}),
                        ("factor_wc_kernel<DMMA>: 1 warp/cell", {"factor_kernel": 4, "factor_update": 1}),
                        ("factor_wc_kernel<DFMA>: 1 warp/cell", {"factor_kernel": 4, "factor_update": 0}),
                        ("factor_reg_kernel<1>: register-tiled, DFMA (round 1)", {"factor_kernel": 2})):

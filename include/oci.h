@@ -93,8 +93,10 @@ int oci_last_create_error(void);
  * (0 = generic shared-memory elimination, one CTA per cell; 1 = production kernels [default]: for n = 64 the working
  * matrix in shared memory, one pivot warp + one update warp per cell with look-ahead and rank-8 updates on the FP64
  * tensor path (DMMA); for n = 128, 192, 256 register-tiled, clusters of n/64 CTAs; 2 = the register-tiled kernel also
- * for n = 64; 4 = n = 64 with ONE warp per cell, "factor_update" 1 = DMMA [default] or 0 = DFMA rank-8 updates -- the A/B
- * pair behind DESIGN.md's DMMA decision), "solve_mode" (0 = dense
+ * for n = 64; 4 = n = 64 with ONE warp per cell), "factor_update" (n = 64: 2 [default] = DMMA updates, a block that is
+ * not needed soon receives the updates of two consecutive panels in one pass (rank 16); 1 = DMMA, one rank-8 pass per
+ * panel; 0 = DFMA rank-8 updates, "factor_kernel" 4 only -- with 1 the A/B pair behind DESIGN.md's DMMA decision),
+ * "solve_mode" (0 = dense
  * [default]: a2 eliminates the dense A_j with partial pivoting and a5 streams A_j^{-1}, the paper's method;
  * 1 = structured: A_j = D - U V^T with D the 4x4 blocks of Eq. 8b and rank 4G (Eq. 10 / 40b), a2 inverts the
  * blocks and the 4G x 4G capacitance matrix with partial pivoting, a5 applies them -- the same iteration to

@@ -361,7 +361,7 @@ int oci_create(const oci_problem *p, void *workspace_dev, size_t workspace_bytes
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->opt_iterate_kernel = 1;
     ctx->opt_factor_kernel = 1;
-    ctx->opt_factor_update = 1;
+    ctx->opt_factor_update = 2;
     ctx->opt_persistent = -1;
     ctx->opt_st_warp_local = 1;
     ctx->opt_st_fused_setup = 1;

@@ -760,6 +760,10 @@ factor_wc_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_
 // eliminate it, while B applies update p to the other six blocks -- the classic look-ahead of blocked LU. One CTA
 // barrier per panel (A: Z(p) is in shared memory; B: update p - 1 is complete). The critical path of a cell is its
 // 64 pivot steps plus eight one-block updates; six cells (twelve warps) per SM.
+// PAIRED (production): B does not apply every panel's update to every block. Panels are taken in pairs and a block that
+// is not needed soon receives both updates of a pair in ONE pass over its accumulator tiles (wc2_update_blocks16, four
+// DMMAs per tile): 9 block passes per pair instead of 14 -- the accumulator tiles of phase U are 55 % of the kernel's
+// shared-memory wavefronts, the resource it saturates. The schedule is written out in the kernel.
 // Fragment rows: the two 8 x 8 tiles of a 16-row group take the even / the odd rows of the group, so a lane's two
 // tiles are adjacent in a column and accumulators and A fragments move as 16-byte accesses (any permutation of the M
 // dimension of a matrix product is free).
@@ -817,6 +821,68 @@ __device__ __forceinline__ void wc2_update_blocks(double *W, const int (&Jb)[NBL
             dmma884(v.x, v.y, a1[i], zf[I][1]);
             cp[4 * I] = v;
         }
+    }
+}
+
+// The updates of TWO consecutive panels q, p = q + 1 applied to column blocks Jb in one pass over their accumulators
+// (a rank-16 update: four DMMAs per tile instead of two passes of two): with Tq' = block q AFTER update p has been
+// applied to it (pivot rows R_p zeroed, += T_p T_q[R_p, :]) the two updates compose to
+//   W[:, c] <- W[:, c] (rows R_q and R_p zeroed) + Tq' W_old[R_q, c] + T_p W_old[R_p, c],
+// with the ORIGINAL pivot-row entries of both panels as A fragments. zq, zp: B fragments of blocks q (updated) and p;
+// rq0/rq1, rp0/rp1: this lane's pivot rows of the two panels. Two tiles at a time: eight DMMAs, four per accumulator.
+template <int NBLK>
+__device__ __forceinline__ void wc2_update_blocks16(double *W, const int (&Jb)[NBLK], const double (&zq)[8][2], const double (&zp)[8][2],
+                                                    int rq0, int rq1, int rp0, int rp1, int lq, int lg)
+{
+    constexpr int LD = WC2_LD;
+    const int cl = wc2_colmap(lg);
+    double aq0[NBLK], aq1[NBLK], ap0[NBLK], ap1[NBLK];
+#pragma unroll
+    for (int i = 0; i < NBLK; ++i) {
+        const double *col = &W[(8 * Jb[i] + cl) * LD];
+        aq0[i] = col[rq0];
+        aq1[i] = col[rq1];
+        ap0[i] = col[rp0];
+        ap1[i] = col[rp1];
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < NBLK; ++i) {
+        double *col = &W[(8 * Jb[i] + cl) * LD];
+        col[rq0] = 0.0;
+        col[rq1] = 0.0;
+        col[rp0] = 0.0;
+        col[rp1] = 0.0;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < NBLK; ++i) {
+        double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb[i] + cl) * LD + 2 * lq]);
+#pragma unroll
+        for (int I = 0; I < 8; I += 2) {
+            double2 v0 = cp[4 * I], v1 = cp[4 * I + 4];
+            dmma884(v0.x, v0.y, aq0[i], zq[I][0]);
+            dmma884(v1.x, v1.y, aq0[i], zq[I + 1][0]);
+            dmma884(v0.x, v0.y, aq1[i], zq[I][1]);
+            dmma884(v1.x, v1.y, aq1[i], zq[I + 1][1]);
+            dmma884(v0.x, v0.y, ap0[i], zp[I][0]);
+            dmma884(v1.x, v1.y, ap0[i], zp[I + 1][0]);
+            dmma884(v0.x, v0.y, ap1[i], zp[I][1]);
+            dmma884(v1.x, v1.y, ap1[i], zp[I + 1][1]);
+            cp[4 * I] = v0;
+            cp[4 * I + 4] = v1;
+        }
+    }
+}
+
+// B fragments of the eliminated panel in column block `blk`: T[8 I + lg][block column 4 h + lq]
+__device__ __forceinline__ void wc2_load_zf(const double *W, int blk, double (&zf)[8][2], int lq, int lg)
+{
+    constexpr int LD = WC2_LD;
+#pragma unroll
+    for (int I = 0; I < 8; ++I) {
+        zf[I][0] = W[(FR_NB * blk + lq) * LD + 8 * I + lg];
+        zf[I][1] = W[(FR_NB * blk + 4 + lq) * LD + 8 * I + lg];
     }
 }
 
@@ -941,7 +1007,7 @@ __device__ __forceinline__ void wc2_panel(WcPanel &R, double *prow, int *rho, in
     }
 }
 
-template <bool DUMP>
+template <bool DUMP, bool PAIRED>
 __global__ void __launch_bounds__(64)
 factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_cell, double *__restrict__ dumpA, int dump_cell,
                   int /* unused */)
@@ -1007,14 +1073,64 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
             __syncthreads(); // barrier p: Z(p), R(p) visible to B; B has completed update p - 1
             if (sh.sing) { singular = true; break; } // CTA-uniform
 
-            // ================= phase U: rank-8 update of the other 56 columns =================
+            // ================= phase U =================
             const int rk0 = sh.rho[FR_NB * pnl + lq], rk1 = sh.rho[FR_NB * pnl + 4 + lq];
-            double zf[8][2]; // B fragments: T[8 I + lg][panel column 4 h + lq]
-#pragma unroll
-            for (int I = 0; I < 8; ++I) {
-                zf[I][0] = W[(FR_NB * pnl + lq) * LD + 8 * I + lg];
-                zf[I][1] = W[(FR_NB * pnl + 4 + lq) * LD + 8 * I + lg];
+            if (PAIRED) {
+                // Panels are paired (q, p = q + 1), q even, and a block that is not needed soon receives the two updates of
+                // a pair in ONE pass over its accumulators (wc2_update_blocks16): 9 block passes per pair instead of 14,
+                // and the accumulator tiles are what saturates the shared-memory pipe. Who needs what, and when:
+                //   A after barrier p': update p' on block p' + 1 (the look-ahead), which therefore must be current
+                //     through p' - 1 at that barrier;
+                //   B after an even barrier q: the LATE blocks of the pair before (two of its five "other" blocks), then
+                //     update q on block q + 2 (A's look-ahead after barrier p applies update p to it);
+                //   B after an odd barrier p: update p on block q (which makes Tq'), then the pair on its three EARLY other
+                //     blocks p + 2, p + 3, p + 4 (mod 8) -- p + 2 is the one A needs after the next barrier.
+                // The other blocks of a pair are p + 2 .. p + 6 (mod 8): everything but q, p and p + 1. The last pair has
+                // no p + 1: its six other blocks are shared out between the two warps after the loop.
+                const int q = pnl & ~1, pp = q + 1;
+                if (roleA) {
+                    if (pnl + 1 < NPANEL) {
+                        double zf[8][2];
+                        wc2_load_zf(W, pnl, zf, lq, lg);
+                        const int jb[1] = {pnl + 1};
+                        wc2_update_blocks<1>(W, jb, zf, rk0, rk1, lq, lg);
+                        __syncwarp();
+                    }
+                } else if ((pnl & 1) == 0) {
+                    if (q >= 2) { // the late blocks of pair (q - 2, q - 1)
+                        double zq[8][2], zp[8][2];
+                        wc2_load_zf(W, q - 2, zq, lq, lg);
+                        wc2_load_zf(W, q - 1, zp, lq, lg);
+                        const int jb[2] = {(q + 4) & 7, (q + 5) & 7}; // (p' + 5, p' + 6 with p' = q - 1)
+                        wc2_update_blocks16<2>(W, jb, zq, zp, sh.rho[FR_NB * (q - 2) + lq], sh.rho[FR_NB * (q - 2) + 4 + lq],
+                                               sh.rho[FR_NB * (q - 1) + lq], sh.rho[FR_NB * (q - 1) + 4 + lq], lq, lg);
+                        __syncwarp();
+                    }
+                    if (q + 2 < NPANEL) {
+                        double zf[8][2];
+                        wc2_load_zf(W, q, zf, lq, lg);
+                        const int jb[1] = {q + 2};
+                        wc2_update_blocks<1>(W, jb, zf, rk0, rk1, lq, lg);
+                    }
+                } else {
+                    double zp[8][2];
+                    wc2_load_zf(W, pp, zp, lq, lg);
+                    {
+                        const int jb[1] = {q};
+                        wc2_update_blocks<1>(W, jb, zp, rk0, rk1, lq, lg); // block q becomes Tq'
+                        __syncwarp();
+                    }
+                    if (pp + 1 < NPANEL) {
+                        double zq[8][2];
+                        wc2_load_zf(W, q, zq, lq, lg);
+                        const int jb[3] = {(pp + 2) & 7, (pp + 3) & 7, (pp + 4) & 7};
+                        wc2_update_blocks16<3>(W, jb, zq, zp, sh.rho[FR_NB * q + lq], sh.rho[FR_NB * q + 4 + lq], rk0, rk1, lq, lg);
+                    }
+                }
+                continue;
             }
+            double zf[8][2]; // B fragments: T[8 I + lg][panel column 4 h + lq]
+            wc2_load_zf(W, pnl, zf, lq, lg);
             if (pnl + 1 < NPANEL) { // A: the next panel's block only (then straight on to eliminate it); B: the rest
                 if (roleA) {
                     const int jb[1] = {pnl + 1};
@@ -1036,7 +1152,15 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
                 }
             }
         }
-        __syncthreads(); // update 7 complete
+        __syncthreads(); // update 7 complete (PAIRED: block 6 has received update 7)
+        if (PAIRED && !singular) { // the last pair (6, 7) on its six other blocks, three per warp
+            double zq[8][2], zp[8][2];
+            wc2_load_zf(W, 6, zq, lq, lg);
+            wc2_load_zf(W, 7, zp, lq, lg);
+            const int jb[3] = {3 * w, 3 * w + 1, 3 * w + 2};
+            wc2_update_blocks16<3>(W, jb, zq, zp, sh.rho[48 + lq], sh.rho[52 + lq], sh.rho[56 + lq], sh.rho[60 + lq], lq, lg);
+            __syncthreads();
+        }
 
         double *out = Minv + (size_t)cell * n * n;
         if (singular) {
@@ -1711,7 +1835,9 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
     const int threads = two ? 64 : 32;
     const bool dmma = ctx->opt_factor_update != 0;
     const void *fn;
-    if (two) fn = dumpA ? (const void *)factor_wc2_kernel<true> : (const void *)factor_wc2_kernel<false>;
+    if (two) fn = dumpA ? (const void *)factor_wc2_kernel<true, false>
+                        : (ctx->opt_factor_update >= 2 ? (const void *)factor_wc2_kernel<false, true>
+                                                       : (const void *)factor_wc2_kernel<false, false>);
     else fn = dumpA ? (const void *)factor_wc_kernel<true, true>
                     : (dmma ? (const void *)factor_wc_kernel<true, false> : (const void *)factor_wc_kernel<false, false>);
     OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

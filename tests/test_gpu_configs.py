@@ -261,6 +261,7 @@ def test_production_assembly_bit_exact(name, make):
     (8, 8, {"factor_kernel": 0}),      # n = 256, same
     (10, 5, {}),                       # n = 200: not a multiple of 64 -> the generic kernel by default, global scratch
     (16, 1, {"factor_kernel": 0}),     # n = 64, generic kernel, working array in shared memory
+    (16, 1, {"factor_update": 1}),     # n = 64, production kernel with one rank-8 pass per panel (default: panels paired)
     (16, 1, {"factor_kernel": 4}),     # n = 64, one warp per cell (DMMA update)
     (16, 1, {"factor_kernel": 4, "factor_update": 0}),   # n = 64, one warp per cell (DFMA update)
     (16, 1, {"factor_kernel": 2}),     # n = 64, register-tiled cluster-capable kernel
