@@ -178,7 +178,9 @@ int oci_debug_get_matrix(oci_ctx *ctx, int32_t cell, double *A_host);   /* assem
  * (the generic shared-memory kernel) or in solve_mode 1. */
 int oci_debug_get_factor_input(oci_ctx *ctx, int32_t cell, double *A_host);
 int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host);/* what oci_factor stored for j
-                                                                          (OCI_E_UNSUPPORTED in solve_mode 1) */
+                                                                          (OCI_E_UNSUPPORTED in solve_mode 1); also
+                                                                          after an oci_factor that reported singular
+                                                                          cells: zeros for those, A_j^{-1} elsewhere */
 int oci_debug_get_const_rhs(oci_ctx *ctx, double *c_dev);               /* [J][n] c_j of a3 [async]       */
 
 /* Enqueues `count` launches of an empty kernel (one CTA per SM) on the context's stream: the launch floor that the

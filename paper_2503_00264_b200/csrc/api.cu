@@ -199,7 +199,8 @@ int factor_finish(oci_ctx *ctx)
     OCI_CUDA_TRY(ctx, cudaEventElapsedTime(&ms, ctx->evf0, ctx->evf1));
     ctx->last_ms[0] = ms;
     const int info = *factor_info_host(ctx);
-    if (info != 0x7f7f7f7f) return info; // 1-based index of the first singular cell
+    ctx->factor_flagged = info != 0x7f7f7f7f;
+    if (ctx->factor_flagged) return info; // 1-based index of the first singular cell
     ctx->factored = true;
     return 0;
 }
@@ -696,7 +697,7 @@ int oci_debug_get_inverse(oci_ctx *ctx, int32_t cell, double *Ainv_host)
     DeviceGuard guard(ctx->device);
     if (cell < 0 || cell >= ctx->J) return -2;
     if (!Ainv_host) return -3;
-    if (!ctx->factored) return OCI_E_STATE;
+    if (!ctx->factored && !ctx->factor_flagged) return OCI_E_STATE;
     if (ctx->opt_solve_mode == 1) return OCI_E_UNSUPPORTED; // the structured path never forms A_j^{-1}
     const size_t n = ctx->n;
     std::vector<double> tmp(n * n);

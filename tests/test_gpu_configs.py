@@ -308,6 +308,37 @@ def test_pivot_ties_take_the_first_maximal_row():
 # ---------------------------------------------------------------------------------------------------------------
 # Library robustness
 # ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,G", [(16, 1), (8, 4), (6, 8), (8, 8)])   # n = 64, 128, 192, 256: the production factor kernels
+def test_production_kernels_flag_singular_cells_and_go_on(N, G):
+    """A singular cell in the middle of the batch: oci_factor returns the 1-based index of the FIRST bad cell, and the
+    CTA / cluster that met it carries on with its next cells (in the cluster kernel the panel buffers and their
+    mbarrier parities must survive a cell that stops at an arbitrary panel). G = 1: sigma_t is NaN, caught in the first
+    panel; G > 1: one column group of the transfer matrix is NaN, which the pivot search only meets when it reaches
+    that group's columns -- panel 20 of 32 at n = 256, in the third CTA of the cluster."""
+    J, bad = 161, (7, 55, 140)
+    p = W.random_problem(300 + N + G, J, N, G, dt=0.02)
+    p.sigma_t = p.sigma_t.copy()
+    p.transfer = p.transfer.copy()
+    for j in bad:
+        if G == 1:
+            p.sigma_t[j] = np.nan
+        else:
+            p.transfer[j, :, (5 * G) // 8] = np.nan
+    s = _solver(p)
+    assert s.factor() == bad[0] + 1
+    o = _oracle(p)
+    good = [j for j in (0, 6, 8, 40, 54, 56, 73, 106, 139, 141, 160)]
+    for j in good:
+        A = o.assemble_cell(j)
+        assert np.max(np.abs(A @ s.debug_inverse(j) - np.eye(p.n))) < 1e-12 * np.linalg.cond(A), f"cell {j}"
+    for j in bad:
+        assert np.all(s.debug_inverse(j) == 0.0)
+    s.set_dt(0.03)                       # and the next elimination on the same context is sound
+    assert s.factor() == bad[0] + 1
+    A = _oracle(p.with_dt(0.03)).assemble_cell(73)
+    assert np.max(np.abs(A @ s.debug_inverse(73) - np.eye(p.n))) < 1e-12 * np.linalg.cond(A)
+
+
 def test_two_contexts_with_different_shapes_in_one_process():
     import torch
     pa, pb = W.config5(J=600, dt=1e-2), W.config3(J=300)
