@@ -1354,9 +1354,11 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
     extern __shared__ __align__(16) unsigned char p128_smem[];
     P128Shared &sh = *reinterpret_cast<P128Shared *>(p128_smem);
     double *W = sh.W;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
-    const bool roleA = w < P128_AW;
-
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
+    // pivot warps on two of the SM's four sub-partitions (physical warps 0, 1, 4, 5), update warps on the other two: a
+    // DFMA of the pivot chain then never queues behind an update warp's DMMA. w = index within the role (+ 4: update).
+    const bool roleA = (wp & 2) == 0;
+    const int w = ((wp & 1) | ((wp >> 2) << 1)) + (roleA ? 0 : P128_AW);
     for (;;) {
         if (threadIdx.x == 0) { sh.cell = DUMP ? dump_cell : atomicAdd(next_cell, 1); sh.sing = 0; sh.tie = 0; }
         __syncthreads();
@@ -1548,6 +1550,9 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
     extern __shared__ __align__(16) unsigned char cq_smem[];
     CqShared<NQ> &sh = *reinterpret_cast<CqShared<NQ> *>(cq_smem);
     double *W = sh.W;
+    // (roles by warp index: putting the pivot warps on sub-partitions of their own, as in factor_p128_kernel, was measured
+    // slower here -- 8.4 -> 9.6 ms at n = 256, 3.8 -> 4.0 ms at n = 192: three pivot warps per sub-partition, and the update
+    // warps' DMMAs on one or two pipes instead of four)
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
     const int q = (int)cluster_ctarank();
     const int n_clusters = gridDim.x / NQ, cluster_id = blockIdx.x / NQ;
