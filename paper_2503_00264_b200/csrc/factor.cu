@@ -1404,6 +1404,34 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
 
             // ================= phase U: rank-8 update of the other 120 columns =================
             const int rk0 = sh.rho[FR_NB * pnl + lq], rk1 = sh.rho[FR_NB * pnl + 4 + lq];
+            if (pnl + 1 < NPANEL && roleA) {
+                // look-ahead: the next panel's block, pivot warp w its own 32 rows (row tiles 4 w .. 4 w + 3), on the critical
+                // path of the cell: only the B fragments of those four tiles are loaded, all loads before the DMMAs, and
+                // the two dependent DMMAs of a tile are four issue slots apart. Z = T - I explicitly (zeroing the pivot
+                // rows would cost a second pivot-warp barrier).
+                const int Jb = pnl + 1, cl = wc2_colmap(lg);
+                const double a0 = W[(8 * Jb + cl) * LD + rk0], a1 = W[(8 * Jb + cl) * LD + rk1];
+                double z0[4], z1[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int row = 8 * (4 * w + i) + lg;
+                    z0[i] = W[(FR_NB * pnl + lq) * LD + row] - (rk0 == row ? 1.0 : 0.0);
+                    z1[i] = W[(FR_NB * pnl + 4 + lq) * LD + row] - (rk1 == row ? 1.0 : 0.0);
+                }
+                p128_bar_pivot(); // every pivot warp has read the pivot rows of the block
+                double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq + 32 * w]);
+                double2 v[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[i] = cp[4 * i];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) dmma884(v[i].x, v[i].y, a0, z0[i]);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) dmma884(v[i].x, v[i].y, a1, z1[i]);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) cp[4 * i] = v[i];
+                __syncwarp();
+                continue;
+            }
             double zf[16][2]; // B fragments: T[8 I + lg][panel column 4 h + lq]
 #pragma unroll
             for (int I = 0; I < 16; ++I) {
@@ -1411,27 +1439,8 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
                 zf[I][1] = W[(FR_NB * pnl + 4 + lq) * LD + 8 * I + lg];
             }
             if (pnl + 1 < NPANEL) {
-                if (roleA) {
-                    // look-ahead: the next panel's block, pivot warp w its own 32 rows (row tiles 4 w .. 4 w + 3). Z = T - I
-                    // explicitly here (zeroing the pivot rows would cost a second pivot-warp barrier).
-                    const int Jb = pnl + 1, cl = wc2_colmap(lg);
-                    const double a0 = W[(8 * Jb + cl) * LD + rk0], a1 = W[(8 * Jb + cl) * LD + rk1];
-                    p128_bar_pivot(); // every pivot warp has read the pivot rows of the block
-                    double2 *cp = reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]);
-#pragma unroll
-                    for (int I = 0; I < 16; ++I) {
-                        if ((I >> 2) != w) continue;
-                        const int row = 8 * I + lg;
-                        double2 v = cp[4 * I];
-                        dmma884(v.x, v.y, a0, zf[I][0] - (rk0 == row ? 1.0 : 0.0));
-                        dmma884(v.x, v.y, a1, zf[I][1] - (rk1 == row ? 1.0 : 0.0));
-                        cp[4 * I] = v;
-                    }
-                    __syncwarp();
-                } else {
-                    for (int Jb = w - P128_AW; Jb < NPANEL; Jb += P128_THREADS / 32 - P128_AW)
-                        if (Jb != pnl && Jb != pnl + 1) p128_update_block(W, Jb, zf, rk0, rk1, lq, lg);
-                }
+                for (int Jb = w - P128_AW; Jb < NPANEL; Jb += P128_THREADS / 32 - P128_AW)
+                    if (Jb != pnl && Jb != pnl + 1) p128_update_block(W, Jb, zf, rk0, rk1, lq, lg);
             } else { // last panel: the other 15 blocks shared out over all eight warps
                 for (int Jb = w; Jb < NPANEL - 1; Jb += P128_THREADS / 32) p128_update_block(W, Jb, zf, rk0, rk1, lq, lg);
             }
