@@ -550,3 +550,29 @@ def test_dense_resident_auto_applies_to_config2_and_matches_the_per_iteration_ke
     assert ia == ib
     assert a.last_timing(1)[1] < b.last_timing(1)[1]          # one launch per batch instead of one per iteration
     assert rel(a.scalar_flux().cpu().numpy(), b.scalar_flux().cpu().numpy()) < 1e-13
+
+
+@pytest.mark.parametrize("opts", [{}, {"solve_mode": 1}], ids=["dense", "structured"])
+@pytest.mark.parametrize("J,N,G", [(1201, 16, 1), (333, 8, 4), (150, 8, 8)])   # n = 64, 128, 256: the warp-per-cell kernels
+def test_walk_direction_does_not_change_an_iteration(J, N, G, opts):
+    """The streaming iterate kernels walk every CTA's range of cells upwards or downwards depending on the parity of the
+    history slot (the tail of one iteration is still in the L2 when the next one asks for it). A Jacobi iteration does
+    not depend on the order of its cells, so the iterates must be BIT-identical whichever way they were produced: one
+    solver iterates from slot 0 (down, up, down), the other burns one slot first and starts again from the same iterate
+    at slot 1 (up, down, up). Ragged J: the CTAs' ranges and the last group of four cells are ragged in both directions."""
+    p = W.random_problem(400 + J, J, N, G, bc_left=1, bc_right=2)
+    a, b = _solver(p, options=opts), _solver(p, options=opts)
+    assert a.factor() == 0 and b.factor() == 0
+    psi0 = b.angular_flux().clone()
+    b.iterate(1)
+    b.set_iterate(psi0)
+    for l in range(3):
+        a.iterate(1)
+        b.iterate(1)
+        assert np.array_equal(a.angular_flux().cpu().numpy(), b.angular_flux().cpu().numpy()), f"iteration {l + 1}"
+        assert np.array_equal(a.scalar_flux().cpu().numpy(), b.scalar_flux().cpu().numpy()), f"iteration {l + 1}"
+    o = _oracle(p)
+    assert o.factor() == 0
+    o.const_rhs()
+    o.oci_iterate(3)
+    assert rel(a.angular_flux().cpu().numpy(), o.psi) < TOL_ITER
