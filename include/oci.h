@@ -93,7 +93,8 @@ int oci_last_create_error(void);
  * (0 = generic shared-memory elimination, one CTA per cell; 1 = production kernels [default]: for n = 64 the working
  * matrix in shared memory, one pivot warp + one update warp per cell with look-ahead and rank-8 updates on the FP64
  * tensor path (DMMA); for n = 128 the same with one CTA per cell (four pivot warps + four update warps); for n = 192,
- * 256 a thread-block cluster of n/64 CTAs per cell, the working matrix in the cluster's distributed shared memory;
+ * 256 a thread-block cluster per cell, the working matrix in the cluster's distributed shared memory ("factor_cluster"
+ * 0 [default] = as few CTAs as hold it, two at n = 192 and three at n = 256; 1 = n/64 CTAs of 64 columns each);
  * 2 = the register-tiled kernels of round 1, n = 64 .. 256; 4 = n = 64 with ONE warp per cell), "factor_update" (n = 64: 2 [default] = DMMA updates, a block that is
  * not needed soon receives the updates of two consecutive panels in one pass (rank 16); 1 = DMMA, one rank-8 pass per
  * panel; 0 = DFMA rank-8 updates, "factor_kernel" 4 only -- with 1 the A/B pair behind DESIGN.md's DMMA decision),

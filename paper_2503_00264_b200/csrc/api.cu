@@ -457,6 +457,7 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     else if (!strcmp(key, "iterate_ctas_per_sm")) ctx->opt_ctas_per_sm = (int)value;
     else if (!strcmp(key, "factor_kernel")) { ctx->opt_factor_kernel = (int)value; ctx->factored = false; }
     else if (!strcmp(key, "factor_update")) { ctx->opt_factor_update = (int)value; ctx->factored = false; }
+    else if (!strcmp(key, "factor_cluster")) { ctx->opt_factor_cluster = (int)value; ctx->factored = false; }
     else if (!strcmp(key, "refactor_every_step")) ctx->opt_refactor_every_step = (int)value;
     else if (!strcmp(key, "solve_mode")) {
         if (value != 0 && value != 1) return -3;

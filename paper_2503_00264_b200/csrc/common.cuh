@@ -79,7 +79,7 @@ struct oci_ctx {
     bool factored, c_valid, si_valid, phi_valid;
     bool factor_flagged; // the last oci_factor reported singular cells: the other cells' inverses are in place (debug getter)
     // options
-    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering, opt_st_warp_local, opt_st_ct, opt_st_fused_setup;
+    int opt_iterate_kernel, opt_stages, opt_ctas_per_sm, opt_factor_kernel, opt_factor_update, opt_factor_cluster, opt_refactor_every_step, opt_si_lanes, opt_solve_mode, opt_si_sweep, opt_persistent, opt_ordering, opt_st_warp_local, opt_st_ct, opt_st_fused_setup;
     // largest dynamic shared-memory size already granted (cudaFuncSetAttribute) to each kernel this context launches;
     // kept per context (= per device), never in function-local statics
     size_t smem_granted[OCI_SMEM_SLOTS];

@@ -491,23 +491,10 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 // issue slots (~66 cycles) apart, so the warp is bound by the 16.5 cycles a DMMA occupies its sub-partition's pipe.
 // cp: the lane's double2 of tile 0 (tile stride: 4 double2 = 8 rows); zp0 / zp1: the lane's B-fragment entries of tile 0
 // (tile stride 8 doubles).
-// PIPELINED = false: tile after tile, as the compiler emits the plain loop (about a third of the rate). Used where the
-// warp has time to spare and shares its sub-partition with warps of the pivot chain: DMMAs issued back to back keep their
-// DFMAs off the FP64 pipe (n = 192: 4.29 -> 3.89 ms with the owner's update warps unpipelined; n = 256: 10.2 -> 11.7).
-template <int NT, bool PIPELINED = true>
+template <int NT>
 __device__ __forceinline__ void dmma_strip(double2 *cp, const double *zp0, const double *zp1, double a0, double a1)
 {
     static_assert(NT % 4 == 0, "tiles are processed four at a time");
-    if (!PIPELINED) {
-#pragma unroll 4
-        for (int I = 0; I < NT; ++I) {
-            double2 v = cp[4 * I];
-            dmma884(v.x, v.y, a0, zp0[8 * I]);
-            dmma884(v.x, v.y, a1, zp1[8 * I]);
-            cp[4 * I] = v;
-        }
-        return;
-    }
     double2 v[2][4];
     double z0[2][4], z1[2][4];
 #pragma unroll
@@ -1472,12 +1459,16 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
 }
 
 // ============================================================================================================
-// n = 64 NQ, NQ = 3, 4 (n = 192, 256: config 4, Table 2 with S32): a cluster of NQ CTAs per cell, working matrix in the
+// n = 64 NS, NS = 3, 4 (n = 192, 256: config 4, Table 2 with S32): a cluster of NQ CTAs per cell, working matrix in the
 // DISTRIBUTED shared memory of the cluster.
 // ============================================================================================================
-// The design of factor_p128_kernel where one working matrix (532 KB at n = 256) no longer fits one SM: CTA q of the
-// cluster keeps columns [64 q, 64 q + 64) (133 KB, column-major, leading dimension n + 4). Panel p (8 columns) belongs to
-// CTA p / 8: its n / 32 pivot warps (one row per lane) eliminate it out of their own shared memory exactly as in the
+// The design of factor_p128_kernel where one working matrix (532 KB at n = 256) no longer fits one SM: the n / 8 column
+// blocks are dealt out in contiguous runs to the NQ CTAs of a cluster (cq_bstart), each keeping its columns column-major
+// with leading dimension n + 4. NQ is as small as the shared memory allows -- two CTAs of 12 blocks at n = 192 (151 KB),
+// three of 10, 11, 11 at n = 256 (183 KB) -- because a cell's time is its chain of n pivot steps whatever the number of
+// SMs behind it, and the fewer SMs a cell takes the more cells are in flight (74 / 45 clusters on 148 SMs against 45 /
+// 33 with n / 64 CTAs of eight blocks: config 4 8.4 -> 7.1 ms, n = 192 3.8 -> 2.9 ms). Panel p (8 columns) belongs to
+// the CTA that holds its block: its n / 32 pivot warps (one row per lane) eliminate it out of their own shared memory exactly as in the
 // n = 128 kernel -- nothing in a pivot step leaves the SM. The eliminated panel T (n x 8), the pivot rows R and the
 // singular flag then travel ONCE to every other CTA of the cluster: the owner writes them to its own panel buffer and
 // one thread issues a bulk asynchronous copy (cp.async.bulk shared::cta -> shared::cluster, completion on the
@@ -1492,19 +1483,23 @@ factor_p128_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *nex
 // its update p, so the phase of every barrier is a function of the panel count alone).
 constexpr int CQ_THREADS = 384; // 12 warps: the first n / 32 are pivot warps when the CTA owns the panel
 
-template <int NQ> struct CqPanelBuf {
-    double T[FR_NB][64 * NQ + 4]; // [panel column][row]
+template <int NS> struct CqPanelBuf { // NS = n / 64
+    double T[FR_NB][64 * NS + 4]; // [panel column][row]
     int R[FR_NB];
     int sing, pad[7];
 };
 
-template <int NQ> struct CqShared {
-    double W[64 * (64 * NQ + 4)];     // [local column][row]
-    CqPanelBuf<NQ> pb[2];             // [panel parity]
-    P128Slot slot[2][2 * NQ];         // [step parity][pivot warp]
+// column blocks [cq_bstart(q), cq_bstart(q + 1)) of the NB = n / 8 belong to CTA q of a cluster of NQ
+__host__ __device__ constexpr int cq_bstart(int q, int NB, int NQ) { return (q * NB) / NQ; }
+
+template <int NS, int NQ> struct CqShared { // n = 64 NS, cluster of NQ CTAs
+    static constexpr int MAXB = (8 * NS + NQ - 1) / NQ; // column blocks per CTA (at most)
+    double W[8 * MAXB * (64 * NS + 4)]; // [local column][row]
+    CqPanelBuf<NS> pb[2];             // [panel parity]
+    P128Slot slot[2][2 * NS];         // [step parity][pivot warp]
     uint64_t tfull[2];                // panel buffer `parity` holds panel p
     uint64_t tempty[2];               // every peer has finished reading panel buffer `parity`
-    int rho[64 * NQ], rhoinv[64 * NQ];
+    int rho[64 * NS], rhoinv[64 * NS];
     int tie;
 };
 
@@ -1536,10 +1531,10 @@ __device__ __forceinline__ uint32_t cluster_ctarank()
 }
 
 // one whole column block of a CTA's 64 columns by one warp: pivot rows read, zeroed, n / 8 row tiles updated
-template <int NQ>
-__device__ __forceinline__ void cq_update_block(double *W, const CqPanelBuf<NQ> &pb, int Jb, int rk0, int rk1, int lq, int lg)
+template <int NS>
+__device__ __forceinline__ void cq_update_block(double *W, const CqPanelBuf<NS> &pb, int Jb, int rk0, int rk1, int lq, int lg)
 {
-    constexpr int n = 64 * NQ, LD = n + 4;
+    constexpr int n = 64 * NS, LD = n + 4;
     const int cl = wc2_colmap(lg);
     double *a0p = &W[(8 * Jb + cl) * LD + rk0], *a1p = &W[(8 * Jb + cl) * LD + rk1];
     const double a0 = *a0p, a1 = *a1p;
@@ -1550,14 +1545,15 @@ __device__ __forceinline__ void cq_update_block(double *W, const CqPanelBuf<NQ> 
     dmma_strip<n / 8>(reinterpret_cast<double2 *>(&W[(8 * Jb + cl) * LD + 2 * lq]), &pb.T[lq][lg], &pb.T[4 + lq][lg], a0, a1);
 }
 
-template <int NQ, bool DUMP>
+template <int NS, int NQ, bool DUMP>
 __global__ void __launch_bounds__(CQ_THREADS, 1)
 factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__restrict__ dumpA, int dump_cell)
 {
-    constexpr int n = 64 * NQ, LD = n + 4, NPANEL = n / FR_NB, AW = 2 * NQ, NWARP = CQ_THREADS / 32, UW = NWARP - AW;
+    constexpr int n = 64 * NS, LD = n + 4, NPANEL = n / FR_NB, AW = 2 * NS, NWARP = CQ_THREADS / 32, UW = NWARP - AW;
+    constexpr int MAXB = CqShared<NS, NQ>::MAXB;
     constexpr int SENDER = CQ_THREADS - 32; // lane 0 of the last warp: never on the pivot chain, least update work
     extern __shared__ __align__(16) unsigned char cq_smem[];
-    CqShared<NQ> &sh = *reinterpret_cast<CqShared<NQ> *>(cq_smem);
+    CqShared<NS, NQ> &sh = *reinterpret_cast<CqShared<NS, NQ> *>(cq_smem);
     double *W = sh.W;
     // (roles by warp index: putting the pivot warps on sub-partitions of their own, as in factor_p128_kernel, was measured
     // slower here -- 8.4 -> 9.6 ms at n = 256, 3.8 -> 4.0 ms at n = 192: three pivot warps per sub-partition, and the update
@@ -1565,6 +1561,7 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
     const int q = (int)cluster_ctarank();
     const int n_clusters = gridDim.x / NQ, cluster_id = blockIdx.x / NQ;
+    const int b0 = cq_bstart(q, NPANEL, NQ), nbq = cq_bstart(q + 1, NPANEL, NQ) - b0; // this CTA's column blocks
 
     if (threadIdx.x == 0) {
         mbar_init(&sh.tfull[0], 1);
@@ -1585,25 +1582,27 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
     };
 
     for (int cell = DUMP ? dump_cell : cluster_id; cell < P.J; cell += n_clusters) {
-        // ---- a1: this CTA's 64 columns (16 column blocks of 4) x n rows
+        // ---- a1: this CTA's 8 nbq columns (2 nbq column blocks of 4) x n rows
         {
-            double *Wl = W - (size_t)64 * q * LD; // so that the global column index addresses the local array
-            for (int idx = w; idx < NQ * 16; idx += NWARP)
-                assemble_rows2(P, cell, lane, Wl, LD, 16 * q + (idx & 15), 1 << 20, 64 * (idx >> 4), 1 << 20);
+            double *Wl = W - (size_t)8 * b0 * LD; // so that the global column index addresses the local array
+            for (int idx = w; idx < NS * 2 * nbq; idx += NWARP)
+                assemble_rows2(P, cell, lane, Wl, LD, 2 * b0 + idx % (2 * nbq), 1 << 20, 64 * (idx / (2 * nbq)), 1 << 20);
         }
         __syncthreads();
         if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
-            for (int e = threadIdx.x; e < n * 64; e += CQ_THREADS) dumpA[(size_t)(e / 64) * n + 64 * q + (e & 63)] = W[(e & 63) * LD + e / 64];
+            for (int e = threadIdx.x; e < n * 8 * nbq; e += CQ_THREADS)
+                dumpA[(size_t)(e / (8 * nbq)) * n + 8 * b0 + e % (8 * nbq)] = W[(e % (8 * nbq)) * LD + e / (8 * nbq)];
             break;
         }
 
         unsigned m = 0x7fffffffu; // pivot warps: 0 once row 32 w + lane has been a pivot row (tracked in every CTA)
         bool singular = false;
         for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
-            const int owner = pnl >> 3, lb = pnl & 7, buf = gp & 1;
+            const int buf = gp & 1;
             const uint32_t par = (gp >> 1) & 1;
-            const bool own = q == owner, own_next = pnl + 1 < NPANEL && q == ((pnl + 1) >> 3);
-            CqPanelBuf<NQ> &pb = sh.pb[buf];
+            const bool own = pnl >= b0 && pnl < b0 + nbq, own_next = pnl + 1 >= b0 && pnl + 1 < b0 + nbq;
+            const int lb = pnl - b0; // local index of the panel's block (when this CTA owns it)
+            CqPanelBuf<NS> &pb = sh.pb[buf];
             if (own && w < AW) {
                 // ================= phase P: the owner's pivot warps eliminate the n x 8 panel, one row per lane =========
                 // (its block is up to date: updates < pnl - 1 by the update warps before the last CTA barrier, update
@@ -1646,11 +1645,11 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
 #pragma unroll
                     for (int peer = 0; peer < NQ; ++peer)
                         if (peer != q)
-                            bulk_s2peer(mapa_u32(smem_u32(&pb), peer), &pb, (uint32_t)sizeof(CqPanelBuf<NQ>),
+                            bulk_s2peer(mapa_u32(smem_u32(&pb), peer), &pb, (uint32_t)sizeof(CqPanelBuf<NS>),
                                         mapa_u32(smem_u32(&sh.tfull[buf]), peer));
                     mbar_arrive(&sh.tfull[buf]); // the owner's own copy is already in place
                 } else {
-                    mbar_arrive_expect_tx(&sh.tfull[buf], (uint32_t)sizeof(CqPanelBuf<NQ>));
+                    mbar_arrive_expect_tx(&sh.tfull[buf], (uint32_t)sizeof(CqPanelBuf<NS>));
                 }
                 if (pnl > 0) release_panel_buffer(buf ^ 1); // nobody here reads the previous panel any more (a cell's last
                                                              // panel is released after the loop)
@@ -1670,7 +1669,7 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
             }
             // ================= phase U: this CTA's column blocks =================
             const int rk0 = pb.R[lq], rk1 = pb.R[4 + lq];
-            const int nb = (pnl + 1) & 7; // block of the next panel (when this CTA owns it)
+            const int nb = pnl + 1 - b0; // local index of the next panel's block (when this CTA owns it)
             if (own_next && w < AW) {
                 // look-ahead: the next panel's block, pivot warp w its own 32 rows (row tiles 4 w .. 4 w + 3). Every pivot
                 // warp reads the pivot-row entries of the block, one barrier over the pivot warps, then each warp zeroes
@@ -1686,14 +1685,14 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
                               &pb.T[4 + lq][32 * w + lg], a0, a1);
                 __syncwarp();
             } else if (own_next) {
-                // the update warps while the pivot warps are busy with the next panel: this CTA's other six or seven
+                // the update warps while the pivot warps are busy with the next panel: this CTA's other nbq - 2 or nbq - 1
                 // blocks as half-blocks (n / 2 rows), shared out round-robin (the last warp, which is also the sender,
                 // gets the fewest). The pivot-row entries of a block are read by everybody before anybody stores (named
                 // barrier over the update warps); each warp then zeroes the pivot rows that lie in its own half.
                 const int wi = w - AW;
                 const int s1 = own ? (lb < nb ? lb : nb) : nb, s2 = own ? (lb < nb ? nb : lb) : 99; // skipped blocks, sorted
-                const int nitems = 2 * (own ? 6 : 7);
-                constexpr int MAXIT = (14 + UW - 1) / UW;
+                const int nitems = 2 * (nbq - (own ? 2 : 1));
+                constexpr int MAXIT = (2 * (MAXB - 1) + UW - 1) / UW;
                 const int cl = wc2_colmap(lg);
                 double a0[MAXIT], a1[MAXIT];
                 int jb[MAXIT];
@@ -1719,19 +1718,17 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
                         if ((unsigned)(rk0 - r0) < (unsigned)(n / 2)) col[rk0] = 0.0;
                         if ((unsigned)(rk1 - r0) < (unsigned)(n / 2)) col[rk1] = 0.0;
                         __syncwarp();
-                        dmma_strip<n / 16, NQ == 4>(reinterpret_cast<double2 *>(col + 2 * lq + r0), &pb.T[lq][r0 + lg],
+                        dmma_strip<n / 16>(reinterpret_cast<double2 *>(col + 2 * lq + r0), &pb.T[lq][r0 + lg],
                                                     &pb.T[4 + lq][r0 + lg], a0[sl], a1[sl]);
                     }
                 }
             } else {
-                // nobody here is on the pivot chain: whole blocks, one per warp, on the first eight warps
-                if (w < 8) {
-                    int k = 0;
-                    for (int Jb = 0; Jb < 8; ++Jb) {
-                        if (own && Jb == lb) continue;
-                        if (k == w) cq_update_block<NQ>(W, pb, Jb, rk0, rk1, lq, lg);
-                        k = (k + 1 == 8) ? 0 : k + 1;
-                    }
+                // nobody here is on the pivot chain: whole blocks, one per warp
+                int k = 0;
+                for (int Jb = 0; Jb < nbq; ++Jb) {
+                    if (own && Jb == lb) continue;
+                    if (k == w) cq_update_block<NS>(W, pb, Jb, rk0, rk1, lq, lg);
+                    k = (k + 1 == NWARP) ? 0 : k + 1;
                 }
             }
         }
@@ -1741,15 +1738,16 @@ factor_cq_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__
         double *out = Minv + (size_t)cell * n * n;
         if (singular) {
             if (q == 0 && threadIdx.x == 0) atomicMin(info, cell + 1);
-            for (int e = threadIdx.x; e < 64 * n / 2; e += CQ_THREADS) reinterpret_cast<double2 *>(out + (size_t)64 * q * n)[e] = make_double2(0.0, 0.0);
+            for (int e = threadIdx.x; e < 8 * nbq * n / 2; e += CQ_THREADS)
+                reinterpret_cast<double2 *>(out + (size_t)8 * b0 * n)[e] = make_double2(0.0, 0.0);
             __syncthreads();
             continue;
         }
-        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]; this CTA's columns j = 64 q + jl
-        for (int jl = w; jl < 64; jl += NWARP) {
-            double *col = out + (size_t)sh.rho[64 * q + jl] * n;
+        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]; this CTA's columns j = 8 b0 + jl
+        for (int jl = w; jl < 8 * nbq; jl += NWARP) {
+            double *col = out + (size_t)sh.rho[8 * b0 + jl] * n;
 #pragma unroll
-            for (int s2 = 0; s2 < NQ; ++s2) {
+            for (int s2 = 0; s2 < NS; ++s2) {
                 const double2 v = *reinterpret_cast<const double2 *>(&W[jl * LD + 64 * s2 + 2 * lane]);
                 col[sh.rhoinv[64 * s2 + 2 * lane]] = v.x;
                 col[sh.rhoinv[64 * s2 + 2 * lane + 1]] = v.y;
@@ -1875,14 +1873,14 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
 }
 
 // n = 192, 256: a cluster of NQ CTAs per cell (factor_cq_kernel). dumpA != nullptr: only assemble `dump_cell`.
-template <int NQ, bool DUMP> static int launch_factor_cq_t(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
+template <int NS, int NQ, bool DUMP> static int launch_factor_cq_t(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.blockDim = dim3(CQ_THREADS, 1, 1);
-    cfg.dynamicSmemBytes = sizeof(CqShared<NQ>);
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_cq_kernel<NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)sizeof(CqShared<NQ>)));
+    cfg.dynamicSmemBytes = sizeof(CqShared<NS, NQ>);
+    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_cq_kernel<NS, NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)sizeof(CqShared<NS, NQ>)));
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -1894,19 +1892,28 @@ template <int NQ, bool DUMP> static int launch_factor_cq_t(oci_ctx *ctx, const P
     int n_clusters = 1;
     if (!DUMP) {
         cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_cq_kernel<NQ, DUMP>, &cfg));
+        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_cq_kernel<NS, NQ, DUMP>, &cfg));
         if (n_clusters < 1) n_clusters = 1;
         if (n_clusters > ctx->J) n_clusters = ctx->J;
     }
     cfg.gridDim = dim3(NQ * n_clusters, 1, 1);
-    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_cq_kernel<NQ, DUMP>, P, ctx->Minv, ctx->info, dumpA, dump_cell));
+    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_cq_kernel<NS, NQ, DUMP>, P, ctx->Minv, ctx->info, dumpA, dump_cell));
     return 1;
 }
 
+// n = 192: clusters of two CTAs (12 column blocks each), n = 256: of three (10, 11, 11): as few CTAs per cell as hold the
+// working matrix -- a cell's time is its chain of n pivot steps whatever the number of SMs behind it, so the cells in
+// flight (74 / 45 clusters on 148 SMs; clusters of n / 64 CTAs: 45 / 33) are what counts. factor_cluster = 1 restores
+// clusters of n / 64 CTAs with eight column blocks each.
 static int launch_factor_cq(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
 {
-    if (ctx->n == 192) return dumpA ? launch_factor_cq_t<3, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<3, false>(ctx, P, nullptr, 0);
-    return dumpA ? launch_factor_cq_t<4, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<4, false>(ctx, P, nullptr, 0);
+    const bool wide = ctx->opt_factor_cluster == 1;
+    if (ctx->n == 192) {
+        if (wide) return dumpA ? launch_factor_cq_t<3, 3, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<3, 3, false>(ctx, P, nullptr, 0);
+        return dumpA ? launch_factor_cq_t<3, 2, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<3, 2, false>(ctx, P, nullptr, 0);
+    }
+    if (wide) return dumpA ? launch_factor_cq_t<4, 4, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<4, 4, false>(ctx, P, nullptr, 0);
+    return dumpA ? launch_factor_cq_t<4, 3, true>(ctx, P, dumpA, dump_cell) : launch_factor_cq_t<4, 3, false>(ctx, P, nullptr, 0);
 }
 
 // n = 128, one CTA per cell (factor_p128_kernel). dumpA != nullptr: only assemble `dump_cell` and write the tile there.
