@@ -50,6 +50,7 @@ extern "C" {
 #define OCI_E_UNSUPPORTED (-102)/* problem outside the supported range (N odd, n > OCI_MAX_N, ...) */
 #define OCI_E_STATE (-103)      /* call order violated (e.g. iterate before factor) */
 #define OCI_E_NOMEM (-104)      /* host allocation failed */
+#define OCI_E_TOO_LARGE (-105)  /* oci_flux_residual_static: J * G beyond OCI_STATIC_MAX_PAIRS (its scratch is fixed) */
 
 #define OCI_MAX_N 256           /* largest per-cell system order n = 4*N*G */
 #define OCI_RESID_CAP 65536     /* residual history entries kept per time step */
@@ -193,6 +194,36 @@ int oci_debug_empty_launches(oci_ctx *ctx, int32_t count);
  * which 0 = oci_factor, 1 = oci_iterate / the iterations inside oci_step, 2 = si_iterate / si_step iterations.
  * *launches = kernels launched by that call. [sync] */
 int oci_last_timing(oci_ctx *ctx, int32_t which, double *ms, int64_t *launches);
+
+/* ---- The one entry point that needs no allocation at all ------------------------------------------------------
+ * Every call above works out of the workspace the caller allocated for oci_create. Some callers cannot allocate:
+ * a transport module inside a host application whose memory manager owns the whole GPU and passes the module its
+ * arrays but no allocator, or code on a path where cudaMalloc / cudaFree are off limits because they synchronise the
+ * device and stall the process's other streams (a convergence monitor called between a coupled code's iterations).
+ * For them: a6 + a7 (Eq. 44; the tested quantities of the stop rules, PAPER.md:166-171 and
+ * BASELINE.json) on arrays the caller already has, with no context and no workspace:
+ *     phi[j][g][p] = sum_m w[m] psi[j][g][m][p],   resid[0] = max |phi - phi_prev|,   resid[1] = ||phi - phi_prev||_2
+ * (a NaN anywhere gives resid[0] = +inf, like the residual history). All five arrays are DEVICE pointers on one GPU,
+ * fp64, layouts as at the top of this header; resid_dev holds 2 doubles; phi_dev may be the same array as
+ * phi_prev_dev (update in place), no other overlap. [async] on cuda_stream (a cudaStream_t of that GPU, NULL = legacy
+ * default stream); the arrays must stay alive until the stream has passed the call.
+ *
+ * The kernel's scratch (one partial result per CTA and a counter) lives in a static __device__ array inside the
+ * library, OCI_STATIC_SCRATCH_BYTES on every GPU that loads liboci_b200.so, held until the process exits. The call
+ * itself runs no cudaMalloc, cudaFree or any other allocating routine. Consequences the caller has to know:
+ *  - Limit: J * G <= OCI_STATIC_MAX_PAIRS; anything larger returns OCI_E_TOO_LARGE and launches nothing.
+ *  - The first call on each GPU looks up the array's device address (cudaGetSymbolAddress) and keeps it; make that
+ *    first call before starting any stream capture on the thread.
+ *  - All calls on one GPU share the array. Each call clears the counter it needs on its stream before its kernel, so
+ *    calls that follow one another on a stream (or are otherwise ordered) are fine; two calls whose kernels can run on
+ *    the GPU at the same time (different streams, different threads) race on it and give wrong residuals.
+ * Returns 0, -i for a bad i-th argument (null, not device memory, or on another GPU than psi_dev), OCI_E_TOO_LARGE,
+ * or OCI_E_CUDA (oci_static_last_cuda_error() has the cudaError_t of the calling thread's last such failure). */
+#define OCI_STATIC_MAX_PAIRS (1 << 20)                               /* largest J * G (cells x groups)            */
+#define OCI_STATIC_SCRATCH_BYTES (256 + (OCI_STATIC_MAX_PAIRS / 64) * 16) /* 262400 B of device memory per GPU    */
+int oci_flux_residual_static(int32_t J, int32_t N, int32_t G, const double *w_dev, const double *psi_dev,
+                             const double *phi_prev_dev, double *phi_dev, double *resid_dev, void *cuda_stream);
+int oci_static_last_cuda_error(void);
 
 #ifdef __cplusplus
 }

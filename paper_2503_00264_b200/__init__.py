@@ -15,12 +15,13 @@ from pathlib import Path
 
 from . import build as _build
 
-__all__ = ["OCISolver", "OCIError", "load_library", "declared_symbols", "create_error", "BC_VACUUM", "BC_REFLECTIVE",
-           "BC_PRESCRIBED", "STOP_DPHI_INF", "STOP_PAPER"]
+__all__ = ["OCISolver", "OCIError", "load_library", "declared_symbols", "create_error", "flux_residual_static",
+           "STATIC_MAX_PAIRS", "BC_VACUUM", "BC_REFLECTIVE", "BC_PRESCRIBED", "STOP_DPHI_INF", "STOP_PAPER"]
 
 BC_VACUUM, BC_REFLECTIVE, BC_PRESCRIBED = 0, 1, 2
 STOP_DPHI_INF, STOP_PAPER = 0, 1
 RESID_CAP = 65536
+STATIC_MAX_PAIRS = 1 << 20  # OCI_STATIC_MAX_PAIRS: largest J * G flux_residual_static takes
 
 _dptr = C.c_void_p
 _i32, _i64, _f64 = C.c_int32, C.c_int64, C.c_double
@@ -63,6 +64,8 @@ _SIGNATURES = {
     "oci_debug_get_const_rhs": (C.c_int, [_dptr, _dptr]),
     "oci_debug_empty_launches": (C.c_int, [_dptr, _i32]),
     "oci_last_timing": (C.c_int, [_dptr, _i32, C.POINTER(_f64), C.POINTER(_i64)]),
+    "oci_flux_residual_static": (C.c_int, [_i32, _i32, _i32, _dptr, _dptr, _dptr, _dptr, _dptr, _dptr]),
+    "oci_static_last_cuda_error": (C.c_int, []),
 }
 
 
@@ -97,6 +100,36 @@ class OCIError(RuntimeError):
         msg = load_library().oci_strerror(code).decode()
         super().__init__(f"{fn} failed: {code} ({msg})" + (f", cudaError {cuda}" if cuda else ""))
         self.code, self.cuda = code, cuda
+
+
+def flux_residual_static(psi, w, phi_prev, phi_out, resid_out, stream=None) -> None:
+    """oci_flux_residual_static: phi = sum_m w_m psi_m and the residuals max |phi - phi_prev|, ||phi - phi_prev||_2 for
+    arrays the caller holds, without a solver object and without a workspace.
+
+    This is the library's one call for users who cannot allocate device memory: a module living inside an application
+    whose memory pool owns the GPU, or code that must not call cudaMalloc / cudaFree because those stall every stream
+    of the process. The kernel's scratch is a fixed array inside liboci_b200.so (about 256 KB per GPU), so the call --
+    and this wrapper, which only passes pointers -- allocates nothing: `phi_out` [J][G][4] and `resid_out` [2] are the
+    caller's, fp64, contiguous, on the GPU of `psi` [J][G][N][4]; `phi_out` may be `phi_prev`. J * G is limited to
+    STATIC_MAX_PAIRS (OCIError -105 beyond it). The first call on a GPU fetches the array's address; make it before
+    any stream capture. Calls on one GPU share the array: keep them ordered (one stream), never concurrent.
+    Asynchronous on `stream` (default: torch's current stream on that GPU)."""
+    import torch
+
+    lib = load_library()
+    if psi.dim() != 4 or psi.shape[3] != 4:
+        raise ValueError("psi must be [J][G][N][4]")
+    J, G, N = int(psi.shape[0]), int(psi.shape[1]), int(psi.shape[2])
+    for name, t, numel in (("psi", psi, J * G * N * 4), ("w", w, N), ("phi_prev", phi_prev, J * G * 4),
+                           ("phi_out", phi_out, J * G * 4), ("resid_out", resid_out, 2)):
+        if t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != numel or t.device != psi.device:
+            raise ValueError(f"{name}: expected a contiguous fp64 tensor of {numel} elements on {psi.device}")
+    if stream is None:
+        stream = torch.cuda.current_stream(psi.device)
+    code = lib.oci_flux_residual_static(J, N, G, w.data_ptr(), psi.data_ptr(), phi_prev.data_ptr(), phi_out.data_ptr(),
+                                        resid_out.data_ptr(), stream.cuda_stream)
+    if code != 0:
+        raise OCIError("oci_flux_residual_static", code, int(lib.oci_static_last_cuda_error()))
 
 
 class OCISolver:

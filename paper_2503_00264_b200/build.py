@@ -16,7 +16,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "liboci_b200.so"
-SOURCES = ["api.cu", "factor.cu", "iterate.cu", "si.cu", "structured.cu"]
+SOURCES = ["api.cu", "factor.cu", "iterate.cu", "si.cu", "structured.cu", "noalloc.cu"]
 HEADERS = [CSRC / "common.cuh", HERE.parent / "include" / "oci.h"]
 
 NVCC_FLAGS = [

@@ -440,6 +440,7 @@ const char *oci_strerror(int code)
     case OCI_E_UNSUPPORTED: return "problem outside the supported range";
     case OCI_E_STATE: return "call order violated";
     case OCI_E_NOMEM: return "host allocation failed";
+    case OCI_E_TOO_LARGE: return "J * G exceeds OCI_STATIC_MAX_PAIRS: the no-allocation entry point has a fixed scratch array";
     default: return code > 0 ? "singular cell matrix (value = 1-based cell index)" : "invalid argument (value = -index)";
     }
 }
