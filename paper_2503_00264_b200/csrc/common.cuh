@@ -83,6 +83,10 @@ struct oci_ctx {
     // largest dynamic shared-memory size already granted (cudaFuncSetAttribute) to each kernel this context launches;
     // kept per context (= per device), never in function-local statics
     size_t smem_granted[OCI_SMEM_SLOTS];
+    // production factor kernel whose attributes are set and whose occupancy-derived grid is known (factor.cu): with
+    // refactor_every_step the factor launch is on every step's critical path, so this host work is done once
+    const void *factor_fn;
+    int factor_grid;
     // timing
     cudaEvent_t ev0, ev1;
     cudaEvent_t evf0, evf1;        // bracket the factor launch (own pair: a step enqueues factor + iterations before it syncs)

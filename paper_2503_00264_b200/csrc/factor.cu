@@ -636,7 +636,7 @@ factor_wc_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next_
                     const unsigned b2 = __ballot_sync(FULL, cand);
                     src = b2 ? __ffs(b2) - 1 : 0;
                 }
-                if (mhi == 0u || mhi >= 0x7ff00000u) bad = true; // zero / denormal / inf / NaN pivot (or no unused row)
+                if (mhi == 0u || mhi >= 0x7ff00000u) bad = true; // pivot with a zero high word (0, or a denormal below 2^-1042), inf, NaN, or no unused row
                 const int esrc = (eball >> src) & 1;
                 if (lane == src) {
                     double2 *dst = reinterpret_cast<double2 *>(sh.prow[b & 1]);
@@ -767,6 +767,7 @@ struct Wc2Shared {
     double prow[2][FR_NB + 2];     // [step parity]: the pivot row of the current step as it stands, then 1 / pivot
     int rho[64], rhoinv[64];
     int cell, sing;
+    unsigned flip;                 // which of the CTA's two warps runs the pivot chain (factor_wc2_kernel)
 };
 
 // Rank-8 update of column block Jb (8 columns) from the panel whose pivot rows are rk0 = R[lq], rk1 = R[4 + lq]:
@@ -916,7 +917,7 @@ __device__ __forceinline__ void wc2_pivot_step(WcPanel &R, double *prow_base, in
         ball = __ballot_sync(FULL, cand && klo == mlo);
     }
     const int src = (__ffs(ball) - 1) & 31;
-    bad |= (mhi - 1u >= 0x7fefffffu) ? 1u : 0u; // zero / denormal / inf / NaN pivot, or no unused row left
+    bad |= (mhi - 1u >= 0x7fefffffu) ? 1u : 0u; // pivot with a zero high word (0 or < 2^-1042), inf, NaN, or no unused row left
     const int esrc = (eball >> src) & 1;
     const bool p0 = lane == src && esrc == 0, p1 = lane == src && esrc != 0;
     const double f0 = R.t0[b], f1 = R.t1[b];
@@ -1004,12 +1005,18 @@ factor_wc2_kernel(ProblemView P, double *__restrict__ Minv, int *info, int *next
     Wc2Shared &sh = *reinterpret_cast<Wc2Shared *>(wc_smem);
     double *W = sh.W;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, lq = lane & 3, lg = lane >> 2;
-    // Role: warp A runs the pivot chain, warp B the updates. The two warps of a CTA sit on neighbouring SM
+    // Role: warp A runs the pivot chain, warp B the updates. The two warps of a CTA normally sit on neighbouring SM
     // sub-partitions (warp slots 2 k, 2 k + 1: measured); alternating the roles with bit 2 of the slot puts the six A
-    // warps of an SM on all four schedulers instead of two.
-    unsigned slot;
-    asm("mov.u32 %0, %%warpid;" : "=r"(slot));
-    const bool roleA = ((slot ^ (slot >> 2)) & 1u) == 0u;
+    // warps of an SM on all four schedulers instead of two. %warpid is only a scheduling HINT here: thread 0 reads it
+    // once and the roles follow from the warp index within the CTA, so the two warps take complementary roles wherever
+    // the hardware placed them (the PTX ISA makes no promise about slot numbers).
+    if (threadIdx.x == 0) {
+        unsigned slot;
+        asm volatile("mov.u32 %0, %%warpid;" : "=r"(slot));
+        sh.flip = (slot ^ (slot >> 2)) & 1u;
+    }
+    __syncthreads();
+    const bool roleA = (((unsigned)w ^ sh.flip) & 1u) == 0u;
 
     for (;;) {
         if (threadIdx.x == 0) { sh.cell = DUMP ? dump_cell : atomicAdd(next_cell, 1); sh.sing = 0; }
@@ -1852,14 +1859,21 @@ static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, i
                                                        : (const void *)factor_wc2_kernel<false, false>);
     else fn = dumpA ? (const void *)factor_wc_kernel<true, true>
                     : (dmma ? (const void *)factor_wc_kernel<true, false> : (const void *)factor_wc_kernel<false, false>);
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int grid = 1;
+    if (dumpA || ctx->factor_fn != fn) { // attributes and occupancy once per (context, kernel)
+        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        if (!dumpA) {
+            int per_sm = 0;
+            OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem));
+            grid = (per_sm < 1 ? 1 : per_sm) * ctx->num_sms;
+            if (grid > ctx->J) grid = ctx->J;
+            ctx->factor_fn = fn;
+            ctx->factor_grid = grid;
+        }
+    }
     if (!dumpA) {
-        int per_sm = 0;
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem));
-        grid = (per_sm < 1 ? 1 : per_sm) * ctx->num_sms;
-        if (grid > ctx->J) grid = ctx->J;
+        grid = ctx->factor_grid;
         OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->info + 1, 0, sizeof(int), ctx->stream)); // the cell counter
     }
     int *counter = ctx->info + 1;
@@ -1879,8 +1893,11 @@ template <int NS, int NQ, bool DUMP> static int launch_factor_cq_t(oci_ctx *ctx,
     memset(&cfg, 0, sizeof(cfg));
     cfg.blockDim = dim3(CQ_THREADS, 1, 1);
     cfg.dynamicSmemBytes = sizeof(CqShared<NS, NQ>);
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_cq_kernel<NS, NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)sizeof(CqShared<NS, NQ>)));
+    const void *fn = (const void *)factor_cq_kernel<NS, NQ, DUMP>;
+    const bool known = !DUMP && ctx->factor_fn == fn; // attributes and occupancy once per (context, kernel)
+    if (!known)
+        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_cq_kernel<NS, NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                               (int)sizeof(CqShared<NS, NQ>)));
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -1890,11 +1907,14 @@ template <int NS, int NQ, bool DUMP> static int launch_factor_cq_t(oci_ctx *ctx,
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     int n_clusters = 1;
-    if (!DUMP) {
+    if (known) n_clusters = ctx->factor_grid;
+    else if (!DUMP) {
         cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
         OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_cq_kernel<NS, NQ, DUMP>, &cfg));
         if (n_clusters < 1) n_clusters = 1;
         if (n_clusters > ctx->J) n_clusters = ctx->J;
+        ctx->factor_fn = fn;
+        ctx->factor_grid = n_clusters;
     }
     cfg.gridDim = dim3(NQ * n_clusters, 1, 1);
     OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_cq_kernel<NS, NQ, DUMP>, P, ctx->Minv, ctx->info, dumpA, dump_cell));
@@ -1921,7 +1941,10 @@ static int launch_factor_p128(oci_ctx *ctx, const ProblemView &P, double *dumpA,
 {
     const size_t smem = sizeof(P128Shared);
     const void *fn = dumpA ? (const void *)factor_p128_kernel<true> : (const void *)factor_p128_kernel<false>;
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (dumpA || ctx->factor_fn != fn) { // once per (context, kernel)
+        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (!dumpA) ctx->factor_fn = fn;
+    }
     int grid = 1;
     if (!dumpA) {
         grid = ctx->num_sms;
@@ -1951,14 +1974,20 @@ int launch_factor(oci_ctx *ctx)
     const size_t smem = factor_smem_bytes(n, global_w);
     int grid;
     if (!global_w) {
-        OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_gj_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                               (int)smem));
-        int per_sm = 1;
-        OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_gj_kernel<false>,
-                                                                        FACTOR_THREADS, smem));
-        if (per_sm < 1) per_sm = 1;
-        grid = ctx->num_sms * per_sm;
-        if (grid > ctx->J) grid = ctx->J;
+        const void *fn = (const void *)factor_gj_kernel<false>;
+        if (ctx->factor_fn != fn) { // once per (context, kernel)
+            OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_gj_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)smem));
+            int per_sm = 1;
+            OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_gj_kernel<false>,
+                                                                            FACTOR_THREADS, smem));
+            if (per_sm < 1) per_sm = 1;
+            grid = ctx->num_sms * per_sm;
+            if (grid > ctx->J) grid = ctx->J;
+            ctx->factor_fn = fn;
+            ctx->factor_grid = grid;
+        }
+        grid = ctx->factor_grid;
         factor_gj_kernel<false><<<grid, FACTOR_THREADS, smem, ctx->stream>>>(P, ctx->Minv, nullptr, n + 1, ctx->info);
     } else {
         grid = ctx->num_sms * 4;
