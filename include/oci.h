@@ -146,7 +146,12 @@ int oci_iterate(oci_ctx *ctx, int32_t n_iters);
  * executed-iterations counter once per batch (the only host round-trip).
  * iters_out[0] = iterations performed, iters_out[1] = iterations after which the rule first held (0 if never);
  * resid_out = last tested residual. Either may be NULL. [sync] up to the last residual read; the advance kernel may
- * still be in flight on the stream when the call returns (whatever the caller enqueues next on it is ordered after). */
+ * still be in flight on the stream when the call returns (whatever the caller enqueues next on it is ordered after).
+ * Returns > 0 (first singular cell, as oci_factor) when a1 + a2 ran inside this call and met a bad pivot: the factor is
+ * enqueued together with the first batch of iterations, which then ran on zeroed inverses, so the call resets the
+ * iterate to both time levels = psi_{k-1/2} (the state oci_set_state leaves; psi_{k-1/2}, q and the boundary data are
+ * untouched), recomputes phi, empties the residual history and reports 0 iterations: a retry with another dt starts
+ * from a defined state. */
 int oci_step(oci_ctx *ctx, double tol, int32_t max_iters, int32_t check_every, int32_t stop_rule,
              int32_t advance, int32_t *iters_out, double *resid_out);
 

@@ -4,6 +4,7 @@
 #include "common.cuh"
 #include <nvtx3/nvToolsExt.h> // header-only; ranges show up under nsys / ncu --nvtx, and cost nothing otherwise
 #include <math.h>
+#include <initializer_list>
 #include <new>
 #include <stdlib.h>
 #include <string.h>
@@ -286,9 +287,23 @@ int step_impl(oci_ctx *ctx, int scheme, double tol, int max_iters, int check_eve
                                               ctx->stream));
         OCI_CUDA_TRY(ctx, cudaMemcpyAsync(h_exec, ctx->ctrl, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         OCI_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
-        if (factor_pending) { // a singular cell: the iterations of this batch ran on a zeroed block; report it
+        if (factor_pending) {
             factor_pending = false;
-            if ((r = factor_finish(ctx)) != 0) return r;
+            if ((r = factor_finish(ctx)) != 0) {
+                // A singular cell: this batch's iterations ran on a zeroed block and both Jacobi buffers, phi and the
+                // residual slots hold their results. Leave a DEFINED state behind instead: the iterate as oci_set_state
+                // leaves it (both time levels = psi_{k-1/2}, which was not touched), its phi, an empty history. A caller
+                // that catches the code and retries with another dt starts from there.
+                int r2 = launch_seed_iterate(ctx);
+                if (r2 < 0) return r2;
+                if ((r2 = launch_scalar_flux(ctx, ctx->psi[ctx->cur], ctx->phi)) < 0) return r2;
+                if ((r2 = reset_history(ctx)) < 0) return r2;
+                ctx->last_ms[which] = 0.0;
+                ctx->last_launches[which] = launches + 2;
+                if (iters_out) { iters_out[0] = 0; iters_out[1] = 0; }
+                if (resid_out) *resid_out = INFINITY;
+                return r;
+            }
         }
         {
             float t = 0.f; // device time of this batch of k launches (kernels only, no flag read)
@@ -453,33 +468,82 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     if (!ctx) return -1;
     DeviceGuard guard(ctx->device);
     if (!key) return -2;
-    if (!strcmp(key, "iterate_kernel")) ctx->opt_iterate_kernel = (int)value;
-    else if (!strcmp(key, "iterate_stages")) ctx->opt_stages = (int)value;
-    else if (!strcmp(key, "iterate_ctas_per_sm")) ctx->opt_ctas_per_sm = (int)value;
-    else if (!strcmp(key, "factor_kernel")) { ctx->opt_factor_kernel = (int)value; ctx->factored = false; }
-    else if (!strcmp(key, "factor_update")) { ctx->opt_factor_update = (int)value; ctx->factored = false; }
-    else if (!strcmp(key, "factor_cluster")) { ctx->opt_factor_cluster = (int)value; ctx->factored = false; }
-    else if (!strcmp(key, "refactor_every_step")) ctx->opt_refactor_every_step = (int)value;
+    // stale factors also means a stale "some cells were singular" record: oci_debug_get_inverse must not serve the
+    // inverses of another dt / another kernel after it
+    auto drop_factors = [&]() { ctx->factored = false; ctx->factor_flagged = false; };
+    auto in = [&](std::initializer_list<int64_t> ok) {
+        for (int64_t v : ok)
+            if (v == value) return true;
+        return false;
+    };
+    if (!strcmp(key, "iterate_kernel")) {
+        if (!in({0, 1})) return -3;
+        ctx->opt_iterate_kernel = (int)value;
+    }
+    else if (!strcmp(key, "iterate_stages")) {
+        if (value < 0 || value > 64) return -3; // 0 = as many as fit
+        ctx->opt_stages = (int)value;
+    }
+    else if (!strcmp(key, "iterate_ctas_per_sm")) {
+        if (value < 0 || value > 8) return -3; // 0 = the kernel's own choice
+        ctx->opt_ctas_per_sm = (int)value;
+    }
+    else if (!strcmp(key, "factor_kernel")) {
+        if (!in({0, 1, 2, 4})) return -3;
+        ctx->opt_factor_kernel = (int)value;
+        drop_factors();
+    }
+    else if (!strcmp(key, "factor_update")) {
+        if (!in({0, 1, 2})) return -3;
+        ctx->opt_factor_update = (int)value;
+        drop_factors();
+    }
+    else if (!strcmp(key, "factor_cluster")) {
+        if (!in({0, 1})) return -3;
+        ctx->opt_factor_cluster = (int)value;
+        drop_factors();
+    }
+    else if (!strcmp(key, "refactor_every_step")) {
+        if (!in({0, 1})) return -3;
+        ctx->opt_refactor_every_step = (int)value;
+    }
     else if (!strcmp(key, "solve_mode")) {
         if (value != 0 && value != 1) return -3;
         if (value == 1 && !st_supported(ctx)) return OCI_E_UNSUPPORTED;
-        if ((int)value != ctx->opt_solve_mode) ctx->factored = false;
+        if ((int)value != ctx->opt_solve_mode) drop_factors();
         ctx->opt_solve_mode = (int)value;
     }
     else if (!strcmp(key, "ordering")) {
         if (value != 0 && value != 1) return -3;
         ctx->opt_ordering = (int)value;
     }
-    else if (!strcmp(key, "st_consumer_threads")) ctx->opt_st_ct = (int)value; // structured pipeline: 128 / 256, 0 = auto
-    else if (!strcmp(key, "st_fused_setup")) { ctx->opt_st_fused_setup = (int)value; if (ctx->opt_solve_mode == 1) ctx->factored = false; }
-    else if (!strcmp(key, "st_warp_local")) ctx->opt_st_warp_local = (int)value; // structured pipeline: 0 = CTA barriers
-    else if (!strcmp(key, "persistent")) ctx->opt_persistent = (int)value; // -1 auto, 0 off, 1 on (structured path)
+    else if (!strcmp(key, "st_consumer_threads")) { // structured pipeline: 128 / 256, 0 = auto
+        if (!in({0, 128, 256})) return -3;
+        ctx->opt_st_ct = (int)value;
+    }
+    else if (!strcmp(key, "st_fused_setup")) {
+        if (!in({0, 1})) return -3;
+        ctx->opt_st_fused_setup = (int)value;
+        if (ctx->opt_solve_mode == 1) drop_factors();
+    }
+    else if (!strcmp(key, "st_warp_local")) { // structured pipeline: 0 = CTA barriers
+        if (!in({0, 1})) return -3;
+        ctx->opt_st_warp_local = (int)value;
+    }
+    else if (!strcmp(key, "persistent")) { // -1 auto, 0 off, 1 on (structured path)
+        if (!in({-1, 0, 1})) return -3;
+        ctx->opt_persistent = (int)value;
+    }
     else if (!strcmp(key, "si_sweep")) {
         if (value != 0 && value != 1) return -3;
         if ((int)value != ctx->opt_si_sweep) ctx->si_valid = false; // the sweep-order arrays change layout
         ctx->opt_si_sweep = (int)value;
     }
-    else if (!strcmp(key, "si_lanes")) { ctx->opt_si_lanes = (int)value; ctx->si_valid = false; }
+    else if (!strcmp(key, "si_lanes")) {
+        if (!in({0, 4, 8, 16})) return -3; // 0 = default (8)
+        ctx->opt_si_lanes = (int)value;
+        ctx->si_valid = false;
+    }
     else return -2;
     return 0;
 }
@@ -492,6 +556,7 @@ int oci_set_dt(oci_ctx *ctx, double dt)
     if (dt != ctx->dt) {
         ctx->dt = dt;
         ctx->factored = false;
+        ctx->factor_flagged = false;
         ctx->si_valid = false;
         ctx->c_valid = false;
     }

@@ -80,6 +80,67 @@ def test_factor_flags_singular_cell():
     assert s.factor() == 8  # 1-based index of the first bad cell
 
 
+def test_flagged_factors_are_dropped_with_the_dt_they_belong_to():
+    """After an oci_factor that reported a singular cell the debug getter may read the other cells' inverses; once dt
+    (or the factor kernel) changes, those belong to a matrix that no longer exists: OCI_E_STATE until the next factor."""
+    from paper_2503_00264_b200 import OCIError
+    p = W.random_problem(21, 12, 4, 1)
+    p.sigma_t = p.sigma_t.copy()
+    p.sigma_t[7] = np.nan
+    s = _solver(p)
+    assert s.factor() == 8
+    assert np.all(np.isfinite(s.debug_inverse(3)))
+    s.set_dt(p.dt * 0.5)
+    with pytest.raises(OCIError) as e:
+        s.debug_inverse(3)
+    assert e.value.code == -103
+    assert s.factor() == 8
+    s.set_option("factor_kernel", 0)
+    with pytest.raises(OCIError) as e:
+        s.debug_inverse(3)
+    assert e.value.code == -103
+
+
+def test_step_that_meets_a_singular_cell_leaves_a_defined_state():
+    """oci_step enqueues the factor with its first batch of iterations; when the factor flags a cell the call must not
+    hand back whatever those iterations wrote: iterate = both time levels of psi_{k-1/2}, its phi, empty history."""
+    from paper_2503_00264_b200 import OCIError
+    p = W.random_problem(23, 40, 4, 2, bc_left=W.BC_REFLECTIVE)
+    p.sigma_t = p.sigma_t.copy()
+    p.sigma_t[17] = np.nan
+    s = _solver(p)
+    edge = s.get_state().cpu().numpy()
+    for _ in range(2):  # the same answer and the same state on a retry
+        with pytest.raises(OCIError) as e:
+            s.step(tol=1e-9, max_iters=50, check_every=5)
+        assert e.value.code == 18
+        psi = s.angular_flux().cpu().numpy()
+        assert np.array_equal(psi[..., 0:2], edge) and np.array_equal(psi[..., 2:4], edge)
+        phi = s.scalar_flux().cpu().numpy()
+        assert np.allclose(phi, np.einsum("m,jgmp->jgp", p.w, psi), rtol=0, atol=1e-13 * max(np.abs(psi).max(), 1.0))
+        assert np.array_equal(s.get_state().cpu().numpy(), edge)
+        assert len(s.residual_history(0)) == 0
+
+
+def test_option_values_outside_their_range_are_refused():
+    from paper_2503_00264_b200 import OCIError
+    s = _solver(W.random_problem(22, 9, 4, 1))
+    bad = {"factor_kernel": [3, 5, -1], "factor_update": [3, -1], "factor_cluster": [2], "st_consumer_threads": [64, 512],
+           "st_warp_local": [2], "st_fused_setup": [-1], "refactor_every_step": [2], "persistent": [2, -2],
+           "iterate_kernel": [2], "si_lanes": [3, 32], "solve_mode": [2], "ordering": [2], "si_sweep": [2],
+           "iterate_stages": [-1], "iterate_ctas_per_sm": [9]}
+    for key, values in bad.items():
+        for v in values:
+            with pytest.raises(OCIError) as e:
+                s.set_option(key, v)
+            assert e.value.code == -3, (key, v)
+    with pytest.raises(OCIError) as e:
+        s.set_option("no_such_key", 0)
+    assert e.value.code == -2
+    for key, v in [("factor_kernel", 4), ("factor_update", 0), ("si_lanes", 16), ("persistent", -1), ("iterate_stages", 0)]:
+        s.set_option(key, v)  # the documented values still pass
+
+
 @pytest.mark.parametrize("kernel", [1, 0])
 @pytest.mark.parametrize("seed,J,N,G,bl,br", SMALL_CASES)
 def test_oci_per_iteration_parity(seed, J, N, G, bl, br, kernel):
