@@ -70,6 +70,20 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def hbm_roofline(achieved, peak, **extra):
+    """An HBM roofline object. MEASURED_PEAKS.json's hbm_gbs is a COPY bandwidth (half reads, half writes); the iterate
+    kernels are 98 % reads and have been measured a few per cent above it with ncu DRAM traffic equal to the algorithmic
+    bytes, so the figure is a yardstick, not a ceiling: a fraction above 1 is flagged here instead of passing silently
+    (well above 1 would mean reuse out of the L2 or a wrong byte count)."""
+    r = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak}
+    r.update(extra)
+    if achieved > peak:
+        r["frac_above_1"] = ("achieved exceeds the copy-measured peak: read-dominated stream against a read+write "
+                             "copy figure; check `traffic` against the algorithmic bytes" if achieved <= 1.2 * peak else
+                             "achieved is more than 1.2 x the measured peak: L2 reuse or a wrong byte count, not HBM speed")
+    return r
+
+
 def source_hash(kernel: str) -> str:
     import hashlib
     h = hashlib.sha256()
@@ -217,7 +231,8 @@ def run_reference(args):
             solves += sample.J * it
     total = sum(step_s)
     value = solves / total
-    desc = f"first {sample.J} of 65536 cells of config 5, one converged time step per timed step, dt cycling {SWEEP}"
+    which = "all" if sample.J == full.J else f"first {sample.J} of"
+    desc = f"{which} {full.J} cells of config 5, one converged time step per timed step, dt cycling {SWEEP}"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
@@ -366,10 +381,9 @@ def run_ours(args):
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     wl = "config5"
     tr, tr_note = ncu_traffic("oci_iterate_wpc_kernel", wl)
-    roofline = {"bound": "hbm", "kernel": "oci_iterate_wpc_kernel<2,0>", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": tr, "traffic_source": tr_note,
-                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": launch_ms,
-                "kernel_share_of_step": kernel_ms_total / ms_total}
+    roofline = hbm_roofline(achieved, peak, kernel="oci_iterate_wpc_kernel<2,0>", traffic=tr, traffic_source=tr_note,
+                            peak_source=peak_src, algorithmic_bytes_per_launch=alg_bytes, avg_launch_ms=launch_ms,
+                            kernel_share_of_step=kernel_ms_total / ms_total)
     factor_ms = statistics.mean(x for d in per_dt.values() for x in d["factor_ms"])
     exec_flops, alg_flops = 2.0 * n ** 3 * J, (2.0 / 3.0) * n ** 3 * J
     factor_tf = exec_flops / (factor_ms * 1e-3) / 1e12
@@ -513,7 +527,7 @@ def run_per_config(device, peak):
                 us = row[key + "_us_per_iteration"]
                 if p.J * p.n * p.n * 8 > (126 << 20):     # factors exceed the L2: HBM roofline
                     gbs = algorithmic_bytes_per_cell_solve(p.n, p.G) * p.J / (us * 1e-6) / 1e9
-                    row["oci_dense_roofline"] = {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak}
+                    row["oci_dense_roofline"] = hbm_roofline(gbs, peak)
                 else:
                     row["oci_dense_iteration_over_launch_floor"] = us / floor
                 fl = 2.0 * p.n ** 3 * p.J
@@ -651,7 +665,8 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--cpu-cells", type=int, default=65536, help="cells of the cpu_baseline sample")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="minimum host time spent on the cpu_baseline sample")
-    ap.add_argument("--ref-cells", type=int, default=8192, help="cells per step of --impl reference")
+    ap.add_argument("--ref-cells", type=int, default=65536,
+                    help="cells per step of --impl reference (default: all of config 5, the workload of the GPU arm)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-si", action="store_true", help="skip the SI comparator leg (profiling runs)")
     ap.add_argument("--quick", action="store_true",
