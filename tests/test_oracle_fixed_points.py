@@ -70,6 +70,46 @@ def test_one_oci_iteration_is_block_jacobi_of_the_global_system():
     np.testing.assert_allclose(got, want, rtol=0, atol=1e-13 * np.abs(want).max())
 
 
+@pytest.mark.parametrize("bc_left,bc_right", [(W.BC_REFLECTIVE, W.BC_VACUUM), (W.BC_PRESCRIBED, W.BC_REFLECTIVE)])
+def test_one_si_iteration_is_a_sweep_with_every_group_lagged(bc_left, bc_right):
+    """The SI twin of the pin above (Eq. 42-45; Alg. 1): ONE iteration solves the streaming + removal
+    operator L_c + L_b for every (g, m) with the whole scattering source -- all groups, the group's own included -- and
+    the mirror ordinate of a reflective face taken from the OLD iterate (readings A12 and "group-Jacobi").
+    A group-Gauss-Seidel sweep or a mirror from the current sweep reaches the same fixed point but fails this test.
+    Built from Eq. 3 only: M(transfer) - M(0) is the scattering operator; in M(0) the only coupling between two
+    different ordinates is the reflective mirror term."""
+    import copy
+    from pins import global_system, idx
+    p = W.random_problem(31, J=4, N=4, G=3, bc_left=bc_left, bc_right=bc_right)
+    M, rhs = global_system(p, p.q, p.psi0)
+    p0 = copy.copy(p)
+    p0.transfer = np.zeros_like(p.transfer)
+    M0, rhs0 = global_system(p0, p.q, p.psi0)
+    assert np.array_equal(rhs, rhs0)
+    S = M0 - M                                   # scattering (+ fission) moved to the right-hand side
+    assert np.abs(S).max() > 0
+    ordinate = (np.arange(M.shape[0]) // 4) % p.N
+    mirror = np.where(ordinate[:, None] != ordinate[None, :], M0, 0.0)
+    assert np.count_nonzero(mirror) == 2 * p.G * (p.N // 2)   # one face: N/2 incoming ordinates x 2 time levels x G
+    L = M0 - mirror                              # L_c + L_b: what the sweep inverts, ordinate by ordinate
+    rng = np.random.default_rng(1)
+    x0 = rng.uniform(0, 1, size=M.shape[0])
+    want = np.linalg.solve(L, S @ x0 + rhs - mirror @ x0)
+    o = oracle.Oracle(p)
+    o.set_iterate(x0)
+    got = o.si_iterate(1).reshape(-1)
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-13 * np.abs(want).max())
+    # and the variants this pin is there to exclude are really different iterations on this problem
+    scale = np.abs(want).max()
+    assert np.abs(np.linalg.solve(M0, S @ x0 + rhs) - want).max() > 1e-6 * scale   # mirror from the new sweep
+    group = (np.arange(M.shape[0]) // (4 * p.N)) % p.G
+    x = x0.copy()                                                                  # group Gauss-Seidel
+    for g in range(p.G):
+        rows = np.flatnonzero(group == g)
+        x[rows] = np.linalg.solve(L[np.ix_(rows, rows)], (S @ x + rhs - mirror @ x0)[rows])
+    assert np.abs(x - want).max() > 1e-6 * scale
+
+
 def test_rule1_controls_false_convergence():
     """Eq. 12-13: with rho close to 1, rule 1 ends closer to the fixed point than rule 0."""
     p = W.config2(dt=1.0, J=96)       # thin cells, c = 0.9: slow OCI convergence
