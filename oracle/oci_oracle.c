@@ -116,9 +116,8 @@ int orc_gepp_factor(int n, double *A, int *piv)
         for (int i = k + 1; i < n; ++i) {
             double l = A[(size_t)i * n + k] / d;
             A[(size_t)i * n + k] = l;
-            if (l != 0.0)
-                for (int c = k + 1; c < n; ++c)
-                    A[(size_t)i * n + c] -= l * A[(size_t)k * n + c];
+            for (int c = k + 1; c < n; ++c)
+                A[(size_t)i * n + c] -= l * A[(size_t)k * n + c];
         }
     }
     return 0;

@@ -52,34 +52,50 @@ def rel_cell(a, b):
 
 
 def _run_sequence(p, schedule, scheme, solver_options=None, check_every=8, max_iters=4000):
-    """schedule: list of (dt, n_steps). One solver and one oracle walk through the whole sequence; set_dt between the
-    blocks goes through oci_step / si_step (which refactors when the factors are stale). The source of step s is
-    p.source_at_step(s) (config 4's pulse). Returns the per-step iteration counts."""
-    s, o = _solver(p, dt=schedule[0][0], options=solver_options or {}), _oracle(p, dt=schedule[0][0])
+    """schedule: list of (dt, n_steps). One oracle walks through the whole sequence and with it one solver per entry of
+    `solver_options` (a dict, or a list of dicts: e.g. the dense and the structured path side by side, each compared
+    with the ORACLE step by step, never with each other); set_dt between the blocks goes through oci_step / si_step
+    (which refactors when the factors are stale). The source of step s is p.source_at_step(s) (config 4's pulse).
+    Returns the per-step iteration counts."""
+    option_sets = solver_options if isinstance(solver_options, list) else [solver_options or {}]
+    solvers = [_solver(p, dt=schedule[0][0], options=opts) for opts in option_sets]
+    o = _oracle(p, dt=schedule[0][0])
     step = 0
     counts = []
     for dt, n_steps in schedule:
-        s.set_dt(dt)
+        for s in solvers:
+            s.set_dt(dt)
         o.set_dt(dt)
         for _ in range(n_steps):
             q = p.source_at_step(step)
-            s.set_source(q)
             o.set_source(q)
             if scheme == "oci":
-                it_g, conv_g, _ = s.step(tol=p.tol, max_iters=max_iters, check_every=check_every)
                 it_o, _ = o.oci_step(tol=p.tol, max_iters=max_iters)
             else:
-                it_g, conv_g, _ = s.si_step(tol=p.tol, max_iters=max_iters, check_every=check_every)
                 it_o, _ = o.si_step(tol=p.tol, max_iters=max_iters)
-            where = f"{p.name} {scheme} dt={dt:g} step {step}"
-            assert it_g == conv_g == it_o, f"{where}: iterations gpu {it_g} (rule held at {conv_g}), oracle {it_o}"
-            phi_g, st_g = s.scalar_flux().cpu().numpy(), s.get_state().cpu().numpy()
-            assert rel(phi_g, o.phi) < TOL_PHI, where
-            assert rel(st_g, o.psi_prev) < TOL_PHI, where
-            assert rel_cell(phi_g, o.phi) < CELL_TOL_PHI, where
-            counts.append(it_g)
+            for s, opts in zip(solvers, option_sets):
+                s.set_source(q)
+                if scheme == "oci":
+                    it_g, conv_g, _ = s.step(tol=p.tol, max_iters=max_iters, check_every=check_every)
+                else:
+                    it_g, conv_g, _ = s.si_step(tol=p.tol, max_iters=max_iters, check_every=check_every)
+                where = f"{p.name} {scheme} {opts} dt={dt:g} step {step}"
+                assert it_g == conv_g == it_o, f"{where}: iterations gpu {it_g} (rule held at {conv_g}), oracle {it_o}"
+                phi_g, st_g = s.scalar_flux().cpu().numpy(), s.get_state().cpu().numpy()
+                assert rel(phi_g, o.phi) < TOL_PHI, where
+                assert rel(st_g, o.psi_prev) < TOL_PHI, where
+                assert rel_cell(phi_g, o.phi) < CELL_TOL_PHI, where
+            counts.append(it_o)
             step += 1
     return counts
+
+
+# the dense path (the paper's method) and the structured cell solve (SURVEY 8f row f1), each against the oracle
+BOTH_PATHS = [{}, {"solve_mode": 1}]
+
+
+def _paths(scheme):
+    return BOTH_PATHS if scheme == "oci" else None
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -88,7 +104,7 @@ def _run_sequence(p, schedule, scheme, solver_options=None, check_every=8, max_i
 @pytest.mark.parametrize("scheme", ["oci", "si"])
 def test_config1_as_configured(scheme):
     p = W.config1()
-    counts = _run_sequence(p, [(p.dt, p.n_steps)], scheme)
+    counts = _run_sequence(p, [(p.dt, p.n_steps)], scheme, solver_options=_paths(scheme))
     # 17,17,16,16,16 OCI iterations, 6 SI iterations per step (the oracle's own counts are pinned on the CPU)
     assert counts == ([17, 17, 16, 16, 16] if scheme == "oci" else [6] * 5)
 
@@ -101,7 +117,7 @@ def test_config1_as_configured(scheme):
 @pytest.mark.parametrize("dt", [1.0, 0.1, 0.01])
 def test_config2_as_configured(dt, scheme):
     p = W.config2(dt=dt)
-    counts = _run_sequence(p, [(dt, p.n_steps)], scheme, max_iters=20000)
+    counts = _run_sequence(p, [(dt, p.n_steps)], scheme, solver_options=_paths(scheme), max_iters=20000)
     if scheme == "oci" and dt == 1.0:
         assert counts[0] > 500          # the slowly converging regime really is exercised
 
@@ -109,7 +125,7 @@ def test_config2_as_configured(dt, scheme):
 def test_config2_dt_changes_mid_run_through_oci_step():
     """set_dt between blocks of steps of ONE run: oci_step must refactor, the state carries over."""
     p = W.config2(dt=1.0, J=256)
-    _run_sequence(p, [(1.0, 2), (0.1, 3), (0.01, 3), (0.1, 2)], "oci", max_iters=20000)
+    _run_sequence(p, [(1.0, 2), (0.1, 3), (0.01, 3), (0.1, 2)], "oci", solver_options=BOTH_PATHS, max_iters=20000)
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -118,7 +134,7 @@ def test_config2_dt_changes_mid_run_through_oci_step():
 @pytest.mark.parametrize("scheme", ["oci", "si"])
 def test_config3_as_configured(scheme):
     p = W.config3()
-    _run_sequence(p, [(p.dt, p.n_steps)], scheme)
+    _run_sequence(p, [(p.dt, p.n_steps)], scheme, solver_options=_paths(scheme))
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -129,28 +145,32 @@ def test_config3_as_configured(scheme):
 @pytest.mark.parametrize("scheme", ["oci", "si"])
 def test_config4_as_configured_pulsed_source(scheme):
     p = W.config4()
-    counts = _run_sequence(p, [(p.dt, p.n_steps)], scheme)
+    counts = _run_sequence(p, [(p.dt, p.n_steps)], scheme, solver_options=_paths(scheme))
     assert len(counts) == 50
 
 
 @pytest.mark.parametrize("scheme", ["oci", "si"])
 def test_config4b_first_steps_pulsed_source(scheme):
     p = W.config4(v=1000.0)
-    _run_sequence(p, [(p.dt, 3)], scheme)
+    _run_sequence(p, [(p.dt, 3)], scheme, solver_options=_paths(scheme))
 
 
 # ---------------------------------------------------------------------------------------------------------------
-# config 5: the dense path at every dt of the sweep, two steps each, dt changed between the blocks through oci_step
-# (the sequence bench.py times, with factors re-used inside a block)
+# config 5 as BASELINE.json configs[4] writes it: dt in {1, 0.1, 0.01, 1e-3, 1e-4}, 10 steps each, J = 65536, one run,
+# dt changed between the blocks through oci_step (factors re-used inside a block, as bench.py times it). OCI: the
+# dense path (the headline) and the structured cell solve walk the full 50 steps beside one oracle (half a minute of
+# host time); the SI comparator walks the same 50 steps (100-350 sweeps per step at dt = 1 and 0.1).
 # ---------------------------------------------------------------------------------------------------------------
-def test_config5_dense_dt_sweep_as_configured():
+def test_config5_oci_dt_sweep_as_configured_dense_and_structured():
     p = W.config5()
-    _run_sequence(p, [(dt, 2) for dt in p.meta["dt_sweep"]], "oci")
+    counts = _run_sequence(p, [(dt, p.n_steps) for dt in p.meta["dt_sweep"]], "oci", solver_options=BOTH_PATHS)
+    assert len(counts) == 50
 
 
-def test_config5_si_small_dt():
+def test_config5_si_dt_sweep_as_configured():
     p = W.config5()
-    _run_sequence(p, [(1e-3, 2), (1e-4, 2)], "si")
+    counts = _run_sequence(p, [(dt, p.n_steps) for dt in p.meta["dt_sweep"]], "si")
+    assert len(counts) == 50
 
 
 def test_config5_per_cell_scaled_error_of_an_iterate():
@@ -166,6 +186,34 @@ def test_config5_per_cell_scaled_error_of_an_iterate():
         assert rel(psi, o.psi) < TOL_ITER
         assert rel_cell(psi, o.psi) < CELL_TOL_ITER, f"iteration {l + 1}"
         assert rel_cell(s.scalar_flux().cpu().numpy(), o.phi) < CELL_TOL_ITER
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# oci_step_host: the call bench.py's e2e leg is timed through (H2D of q from pinned memory, the step, D2H of phi)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_step_host_matches_the_oracle_and_the_device_getters(scheme):
+    import torch
+    p = W.random_problem(61, 211, 8, 2, bc_left=W.BC_PRESCRIBED, bc_right=W.BC_REFLECTIVE, dt=0.03)
+    s, o = _solver(p), _oracle(p)
+    q_host = torch.empty((p.J, p.G, 4), dtype=torch.float64).pin_memory()
+    phi_host = torch.full((p.J, p.G, 4), float("nan"), dtype=torch.float64).pin_memory()
+    rng = np.random.default_rng(7)
+    for step in range(3):  # a new source every step: the H2D copy must be the one the step uses
+        q = rng.uniform(0.0, 2.0, size=(p.J, p.G, 4))
+        q_host.copy_(torch.from_numpy(q))
+        it_g, conv_g, _ = s.step_host(scheme, q_host, phi_host, tol=1e-9, max_iters=4000, check_every=8)
+        o.set_source(q)
+        it_o, _ = (o.oci_step if scheme == 0 else o.si_step)(tol=1e-9, max_iters=4000)
+        assert it_g == conv_g == it_o, (step, it_g, conv_g, it_o)
+        assert rel(phi_host.numpy(), o.phi) < TOL_PHI
+        assert np.array_equal(phi_host.numpy(), s.scalar_flux().cpu().numpy())  # the same array, copied out
+        assert rel(s.get_state().cpu().numpy(), o.psi_prev) < TOL_PHI
+    # q_host = NULL keeps the source of the last call; phi_host = NULL skips the read-back
+    it_g, _, _ = s.step_host(scheme, None, None, tol=1e-9, max_iters=4000, check_every=8)
+    it_o, _ = (o.oci_step if scheme == 0 else o.si_step)(tol=1e-9, max_iters=4000)
+    assert it_g == it_o
+    assert rel(s.scalar_flux().cpu().numpy(), o.phi) < TOL_PHI
 
 
 # ---------------------------------------------------------------------------------------------------------------
