@@ -633,7 +633,7 @@ def run_table2(args):
 def run_factor_ab(args):
     """The a1 + a2 kernels for n = 64 side by side on config 5 (the DMMA decision): the production
     kernel (two warps per cell, look-ahead, DMMA), the one-warp-per-cell kernel with its rank-8 updates as DMMA and as
-    DFMA (everything else identical), and the register-tiled kernel of round 1. One JSON line."""
+    DFMA (everything else identical), and the generic one-CTA-per-cell kernel. One JSON line."""
     import torch
     from paper_2503_00264_b200 import OCISolver
     p = W.config5(dt=1e-3)
@@ -643,7 +643,7 @@ def run_factor_ab(args):
                        ("factor_wc2_kernel: the same, one rank-8 pass per panel", {"factor_update": 1}),
                        ("factor_wc_kernel<DMMA>: 1 warp/cell", {"factor_kernel": 4, "factor_update": 1}),
                        ("factor_wc_kernel<DFMA>: 1 warp/cell", {"factor_kernel": 4, "factor_update": 0}),
-                       ("factor_reg_kernel<1>: register-tiled, DFMA (round 1)", {"factor_kernel": 2})):
+                       ("factor_gj_kernel: generic, one CTA per cell, DFMA", {"factor_kernel": 0})):
         s = OCISolver(p, options=opts)
         ts = []
         for r in range(4):

@@ -90,13 +90,14 @@ int oci_last_cuda_error(const oci_ctx *ctx);
 int oci_last_create_error(void);
 
 /* Tuning knobs (all optional). Known keys: "iterate_kernel" (0 = plain one-CTA-per-cell, 1 = pipelined
- * bulk-copy streaming kernel [default]), "iterate_stages", "iterate_ctas_per_sm", "factor_kernel"
+ * bulk-copy streaming kernel [default]), "iterate_stages" (depth of its shared-memory ring, 0 [default] = as deep as
+ * fits), "factor_kernel"
  * (0 = generic shared-memory elimination, one CTA per cell; 1 = production kernels [default]: for n = 64 the working
  * matrix in shared memory, one pivot warp + one update warp per cell with look-ahead and rank-8 updates on the FP64
  * tensor path (DMMA); for n = 128 the same with one CTA per cell (four pivot warps + four update warps); for n = 192,
  * 256 a thread-block cluster per cell, the working matrix in the cluster's distributed shared memory ("factor_cluster"
  * 0 [default] = as few CTAs as hold it, two at n = 192 and three at n = 256; 1 = n/64 CTAs of 64 columns each);
- * 2 = the register-tiled kernels of round 1, n = 64 .. 256; 4 = n = 64 with ONE warp per cell), "factor_update" (n = 64: 2 [default] = DMMA updates, a block that is
+ * 4 = n = 64 with ONE warp per cell), "factor_update" (n = 64: 2 [default] = DMMA updates, a block that is
  * not needed soon receives the updates of two consecutive panels in one pass (rank 16); 1 = DMMA, one rank-8 pass per
  * panel; 0 = DFMA rank-8 updates, "factor_kernel" 4 only -- with 1 the A/B pair behind DESIGN.md's DMMA decision),
  * "solve_mode" (0 = dense
@@ -111,9 +112,7 @@ int oci_last_create_error(void);
  * same iterates to rounding), "persistent" (-1 [default] = run a batch of iterations as ONE
  * cooperative launch with grid-wide barriers when the problem is small: structured path <= 8 MB per iteration; dense
  * path when the inverses of ceil(J / SMs) cells fit in one CTA's shared memory, where they then stay for the whole
- * batch; 0 = never, 1 = always (structured path)), "st_warp_local", "st_consumer_threads",
- * "st_fused_setup" (structured path, tuning probes: 0 restores the CTA barriers per batch / 128 or 256 consumer
- * threads per CTA / 0 restores the three set-up launches), "ordering" (structured path only: 0 = block-Jacobi [default], the
+ * batch; 0 = never, 1 = always (structured path)), "ordering" (structured path only: 0 = block-Jacobi [default], the
  * paper's OCI; 1 = red-black: per iteration the even cells, then the odd cells from the new even ones, in place --
  * the block Gauss-Seidel variant PAPER.md:29, 550 names, about half the iterations; SURVEY.md 8(f) row f4;
  * oci_iterate / oci_step return OCI_E_UNSUPPORTED in the dense mode). Returns -2 for an unknown key, -3 for a bad

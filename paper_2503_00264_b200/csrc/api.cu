@@ -112,8 +112,14 @@ size_t carve(oci_ctx *c, unsigned char *base, int J, int N, int G, int num_sms, 
 int reset_history(oci_ctx *ctx)
 {
     OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->ctrl, 0, sizeof(int) * 4, ctx->stream));
-    OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->resid_inf, 0, sizeof(unsigned long long) * OCI_RESID_CAP, ctx->stream));
-    OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->resid_l2, 0, sizeof(double) * OCI_RESID_CAP, ctx->stream));
+    // only the slots that iterations were issued for since the last reset (a step of 20 iterations clears 2 x 160 bytes,
+    // not 2 x 512 KB); every other slot still holds the zero it was given at create or at an earlier reset
+    const size_t dirty = (size_t)(ctx->hist_dirty < OCI_RESID_CAP ? ctx->hist_dirty : OCI_RESID_CAP);
+    if (dirty) {
+        OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->resid_inf, 0, sizeof(unsigned long long) * dirty, ctx->stream));
+        OCI_CUDA_TRY(ctx, cudaMemsetAsync(ctx->resid_l2, 0, sizeof(double) * dirty, ctx->stream));
+    }
+    ctx->hist_dirty = 0;
     ctx->hist_len = 0;
     ctx->hist_has_l2 = 0;
     return 0;
@@ -152,6 +158,7 @@ int one_iteration(oci_ctx *ctx, int scheme, int slot, bool want_l2, bool check_p
 // the one before it and skips itself once the stop rule held (device-side stop). Returns kernels launched.
 int issue_batch(oci_ctx *ctx, int scheme, int slot0, int k, bool want_l2, bool check_between)
 {
+    if (slot0 + k > ctx->hist_dirty) ctx->hist_dirty = slot0 + k;
     if (scheme == 0) { // one cooperative launch for the whole batch, where that applies
         int r = launch_st_multi(ctx, slot0, k, want_l2, check_between);
         if (r != 0) return r;
@@ -484,12 +491,8 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
         if (value < 0 || value > 64) return -3; // 0 = as many as fit
         ctx->opt_stages = (int)value;
     }
-    else if (!strcmp(key, "iterate_ctas_per_sm")) {
-        if (value < 0 || value > 8) return -3; // 0 = the kernel's own choice
-        ctx->opt_ctas_per_sm = (int)value;
-    }
     else if (!strcmp(key, "factor_kernel")) {
-        if (!in({0, 1, 2, 4})) return -3;
+        if (!in({0, 1, 4})) return -3;
         ctx->opt_factor_kernel = (int)value;
         drop_factors();
     }
@@ -516,19 +519,6 @@ int oci_set_option(oci_ctx *ctx, const char *key, int64_t value)
     else if (!strcmp(key, "ordering")) {
         if (value != 0 && value != 1) return -3;
         ctx->opt_ordering = (int)value;
-    }
-    else if (!strcmp(key, "st_consumer_threads")) { // structured pipeline: 128 / 256, 0 = auto
-        if (!in({0, 128, 256})) return -3;
-        ctx->opt_st_ct = (int)value;
-    }
-    else if (!strcmp(key, "st_fused_setup")) {
-        if (!in({0, 1})) return -3;
-        ctx->opt_st_fused_setup = (int)value;
-        if (ctx->opt_solve_mode == 1) drop_factors();
-    }
-    else if (!strcmp(key, "st_warp_local")) { // structured pipeline: 0 = CTA barriers
-        if (!in({0, 1})) return -3;
-        ctx->opt_st_warp_local = (int)value;
     }
     else if (!strcmp(key, "persistent")) { // -1 auto, 0 off, 1 on (structured path)
         if (!in({-1, 0, 1})) return -3;

@@ -70,6 +70,7 @@ struct oci_ctx {
     double *resid_l2;              // [OCI_RESID_CAP] sum of squares
     double *h_resid;               // pinned host, 2 * OCI_RESID_CAP
     int hist_len;                  // iterations recorded since the history was last reset
+    int hist_dirty;                // residual slots [0, hist_dirty) may have been written since they were last zeroed
     int hist_has_l2;
 
     int *ctrl;                     // [4] ctrl[0] = iterations of the current step that really ran (device-side stop)

@@ -128,28 +128,9 @@ factor_gj_kernel(ProblemView P, double *__restrict__ Minv, double *__restrict__ 
     }
 }
 
-// ============================================================================================================
-// Register-tiled, panel-blocked Gauss-Jordan for n = 64 NQ (NQ = 1..4): the production a1 + a2 kernel.
-// ============================================================================================================
-// One cluster of NQ CTAs per cell; CTA q owns the columns [64 q, 64 q + 64), warp w of it the 8-column tile
-// [64 q + 8 w, +8), lane l the rows {64 s + 2 l, 64 s + 2 l + 1}, s < NQ: the whole working matrix W lives in
-// registers (TR x 8 = n / 4 doubles per thread) and is never written anywhere un-eliminated.
-//
-// In-place Gauss-Jordan with implicit row exchange, blocked by panels of NB = 8 columns K = {k_0..k_7}:
-//   phase P  the warp that owns the panel runs the 8 elimination steps on its n x 8 tile alone (warp-level
-//            operations only): pivot row r_b = first row of maximal |W[i][k_b]| among the unused rows (three
-//            redux.sync on the bit pattern), pivot row broadcast by shuffles, W[r][:] /= p, W[i][:] -= f_i W[r][:].
-//            Afterwards column k_b of the tile holds T e_{r_b}, T = the product of the 8 elementary matrices.
-//   phase U  T differs from I only in the columns R = {r_b}, so every other column c becomes
-//            W[:, c] + Z W_old[R, c] with Z = T[:, R] - I[:, R]  (n x 8). The owner publishes Z and R to every
-//            CTA of the cluster (distributed shared memory), each thread that holds a pivot row publishes its
-//            old 8 entries of it (Rrow), and every warp but the owner applies the rank-8 update to its tile.
-// Two barriers per 8 pivots (one cluster-wide, one CTA-wide); Z / Rrow / R are double-buffered so that no third
-// barrier is needed. At the end W[i][j] = A^{-1}[rhoinv[i]][rho[j]] (rho[k] = pivot row of step k).
 namespace cg = cooperative_groups;
 
-constexpr int FR_THREADS = 256;
-constexpr int FR_NB = 8;
+constexpr int FR_NB = 8; // panel width of every blocked factor kernel below
 
 // Branch-free reciprocal: hardware seed (MUFU.RCP64H, relative error 2^-19.9) + one cubic Newton step. Measured on a
 // B200 over 1.3e9 random arguments: at most 1 ulp from the correctly rounded 1 / x (one more quadratic step, two FMAs,
@@ -162,280 +143,6 @@ __device__ __forceinline__ double rcp_nr(double x)
     double e = fma(-x, r, 1.0);
     e = fma(e, e, e);
     return fma(r, e, r);
-}
-
-struct PivotSlot {                 // what a warp's local arg-max winner publishes in a pivot step
-    double row[FR_NB];             // its panel row, scaled by 1 / candidate (column b holds 1 / candidate)
-    unsigned long long key;        // bit pattern of |candidate| (0: this warp has no unused row)
-    int lane;
-    int pad;
-};
-
-template <int NQ> struct FrShared {
-    double Z[2][FR_NB][64 * NQ];          // [buf][b][row]
-    double Pn[FR_NB][64 * NQ];            // [c][row]: the panel, owner's registers -> one row per thread -> back
-    PivotSlot slot[2][FR_THREADS / 32];   // [step parity][warp]
-    double Rrow[2][FR_NB][64];            // [buf][b][local column]
-    int R[2][FR_NB];                      // pivot rows of the panel
-    int sing[2];                          // panel met a zero / non-finite pivot
-    int rho[64 * NQ], rhoinv[64 * NQ];
-};
-
-template <int NQ, bool DUMP>
-__global__ void __launch_bounds__(FR_THREADS, NQ == 1 ? 3 : (NQ == 2 ? 2 : 1))
-factor_reg_kernel(ProblemView P, double *__restrict__ Minv, int *info, double *__restrict__ dumpA, int dump_cell)
-{
-    constexpr int n = 64 * NQ, TR = 2 * NQ, NPANEL = n / FR_NB;
-    extern __shared__ __align__(16) unsigned char fr_smem[];
-    FrShared<NQ> &sh = *reinterpret_cast<FrShared<NQ> *>(fr_smem);
-    constexpr unsigned FULL = 0xffffffffu;
-    cg::cluster_group cluster = cg::this_cluster();
-    const int q = NQ == 1 ? 0 : (int)cluster.block_rank();
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int n_clusters = gridDim.x / NQ, cluster_id = blockIdx.x / NQ;
-    const int N = P.N, G = P.G;
-    unsigned gp = 0; // running panel counter: selects the shared-memory buffer
-
-    auto cluster_barrier = [&]() {
-        if (NQ == 1) __syncthreads();
-        else cluster.sync();
-    };
-
-    for (int cell = DUMP ? dump_cell : cluster_id; cell < P.J; cell += n_clusters) {
-        // ---- a1: assemble the tile, bit-identical to a_entry() (same operations in the same order)
-        double a[TR][8];
-        {
-            const double dx = P.dx[cell];
-            const int p0 = (lane & 1) * 2; // p of row 64 s + 2 lane
-            double Kw[2][NQ], wq[2];       // per column half: transfer entry (per row group) and weight
-            int bmc[2];
-#pragma unroll
-            for (int hc = 0; hc < 2; ++hc) {
-                bmc[hc] = 16 * q + 2 * w + hc;
-                wq[hc] = P.w[bmc[hc] % N];
-            }
-#pragma unroll
-            for (int s = 0; s < NQ; ++s) {
-                const int bm = 16 * s + (lane >> 1), m = bm % N, g = bm / N;
-                const double sig = P.sigma_t[(size_t)cell * G + g], mu = P.mu[m];
-                const double av = __dmul_rn(__dadd_rn(fabs(mu), __dmul_rn(dx, sig)), 0.5);
-                const double gam = __ddiv_rn(dx, __dmul_rn(P.v[g], P.dt));
-                const double h = __dmul_rn(mu, 0.5), hg = __dmul_rn(gam, 0.5), ga = __dadd_rn(gam, av);
-#pragma unroll
-                for (int hc = 0; hc < 2; ++hc) {
-                    const double K = P.transfer[((size_t)cell * G + g) * G + bmc[hc] / N];
-                    Kw[hc][s] = __dmul_rn(__dmul_rn(__dmul_rn(dx, K), 0.25), wq[hc]);
-                }
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int p = p0 + e;
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) {
-                        const int pp = c & 3, hc = c >> 2;
-                        double val = 0.0;
-                        if (bm == bmc[hc]) { // Eq. 8b
-                            const int d = pp - p;
-                            if (d == 0) val = p < 2 ? av : ga;
-                            else if (p == 0 && pp == 1) val = h;
-                            else if (p == 1 && pp == 0) val = -h;
-                            else if (p == 2 && pp == 3) val = h;
-                            else if (p == 3 && pp == 2) val = -h;
-                            else if (d == 2) val = hg;       // (0,2), (1,3)
-                            else if (d == -2) val = -gam;    // (2,0), (3,1)
-                        }
-                        if (p == pp) val = __dsub_rn(val, Kw[hc][s]);
-                        a[2 * s + e][c] = val;
-                    }
-                }
-            }
-        }
-        if (DUMP) { // the assembled tile of the production kernel, row-major, for the bit-exactness test
-#pragma unroll
-            for (int rr = 0; rr < TR; ++rr)
-#pragma unroll
-                for (int c = 0; c < 8; ++c)
-                    dumpA[(size_t)(64 * (rr >> 1) + 2 * lane + (rr & 1)) * n + 64 * q + 8 * w + c] = a[rr][c];
-            return;
-        }
-        bool used_r = false; // row threadIdx.x (the row this thread holds during panel phases) was a pivot row
-        bool singular = false;
-
-        for (int pnl = 0; pnl < NPANEL; ++pnl, ++gp) {
-            const int buf = gp & 1;
-            const bool owner_cta = (pnl >> 3) == q;
-            const bool owner = owner_cta && (pnl & 7) == w;
-            if (owner_cta) {
-                // ================= phase P: the owner CTA eliminates the n x 8 panel, ONE ROW PER THREAD ==============
-                // (a warp holding TR rows per lane would run ~70 + 45 TR dependent instructions per pivot step alone)
-                __syncthreads(); // the previous panel's owner warp has read its panel back from Pn
-                if (owner) {
-#pragma unroll
-                    for (int c = 0; c < 8; ++c)
-#pragma unroll
-                        for (int sq = 0; sq < NQ; ++sq)
-                            *reinterpret_cast<double2 *>(&sh.Pn[c][64 * sq + 2 * lane]) = make_double2(a[2 * sq][c], a[2 * sq + 1][c]);
-                }
-                __syncthreads();
-                const int r = threadIdx.x;             // this thread's row during the panel phase
-                const bool row_on = r < n;
-                double t[FR_NB];
-#pragma unroll
-                for (int c = 0; c < FR_NB; ++c) t[c] = row_on ? sh.Pn[c][r] : 0.0;
-                int Rl[FR_NB];
-                bool bad = false;
-                bool used_p = used_r;
-#pragma unroll
-                for (int b = 0; b < FR_NB; ++b) {
-                    const unsigned long long key =
-                        (used_p || !row_on) ? 0ull : (unsigned long long)__double_as_longlong(fabs(t[b]));
-                    const unsigned khi = (unsigned)(key >> 32);
-                    const unsigned mhi = __reduce_max_sync(FULL, khi);
-                    const double linv = rcp_nr(t[b]);
-                    double scl[FR_NB];
-#pragma unroll
-                    for (int c = 0; c < FR_NB; ++c) scl[c] = (c == b) ? linv : t[c] * linv;
-                    bool cand = !used_p && row_on && khi == mhi;
-                    const unsigned ball = __ballot_sync(FULL, cand);
-                    int src;
-                    if (__popc(ball) == 1) {
-                        src = __ffs(ball) - 1;
-                    } else { // ties in the high word (or no unused row in this warp): low words, then the lowest row
-                        const unsigned klo = (unsigned)key;
-                        const unsigned mlo = __reduce_max_sync(FULL, cand ? klo : 0u);
-                        cand = cand && klo == mlo;
-                        const unsigned b2 = __ballot_sync(FULL, cand);
-                        src = b2 ? __ffs(b2) - 1 : 0;
-                    }
-                    PivotSlot *mys = &sh.slot[b & 1][w];
-                    if (lane == src) {
-#pragma unroll
-                        for (int c = 0; c < FR_NB / 2; ++c)
-                            reinterpret_cast<double2 *>(mys->row)[c] = make_double2(scl[2 * c], scl[2 * c + 1]);
-                        mys->key = key;
-                        mys->lane = lane;
-                    }
-                    __syncthreads(); // the candidates of this step are visible (two slot buffers alternate)
-                    unsigned long long kmax = sh.slot[b & 1][0].key;
-                    int gw = 0;
-#pragma unroll
-                    for (int ww = 1; ww < n / 32; ++ww) { // a tie goes to the lower warp: the lower row
-                        const unsigned long long kk = sh.slot[b & 1][ww].key;
-                        if (kk > kmax) { kmax = kk; gw = ww; }
-                    }
-                    if ((unsigned)(kmax >> 32) == 0u || (unsigned)(kmax >> 32) >= 0x7ff00000u) bad = true;
-                    const PivotSlot *win = &sh.slot[b & 1][gw];
-                    const int lw = win->lane;
-                    Rl[b] = 32 * gw + lw;
-                    double sp[FR_NB];
-#pragma unroll
-                    for (int c = 0; c < FR_NB / 2; ++c) {
-                        const double2 v = reinterpret_cast<const double2 *>(win->row)[c];
-                        sp[2 * c] = v.x;
-                        sp[2 * c + 1] = v.y;
-                    }
-                    const bool is_p = gw == w && lane == lw;
-                    const double f = t[b];
-#pragma unroll
-                    for (int c = 0; c < FR_NB; ++c) {
-                        const double upd = (c == b) ? -f * sp[b] : fma(-f, sp[c], t[c]);
-                        t[c] = is_p ? scl[c] : upd;
-                    }
-                    if (is_p) used_p = true;
-                }
-                // ---- publish Z = T[:, R] - I[:, R], R and the singular flag to every CTA of the cluster; the eliminated
-                // panel goes back to its owner warp through Pn
-#pragma unroll
-                for (int tq = 0; tq < NQ; ++tq) {
-                    FrShared<NQ> *dst = NQ == 1 ? &sh : cluster.map_shared_rank(&sh, tq);
-                    if (row_on) {
-#pragma unroll
-                        for (int b = 0; b < FR_NB; ++b) dst->Z[buf][b][r] = t[b] - (Rl[b] == r ? 1.0 : 0.0);
-                    }
-#pragma unroll
-                    for (int b = 0; b < FR_NB; ++b)
-                        if (threadIdx.x == b) dst->R[buf][b] = Rl[b];
-                    if (threadIdx.x == 0) dst->sing[buf] = bad ? 1 : 0;
-                }
-                if (row_on) {
-#pragma unroll
-                    for (int c = 0; c < FR_NB; ++c) sh.Pn[c][r] = t[c];
-                }
-            }
-            cluster_barrier(); // B1: Z, R, sing of this panel visible everywhere
-
-            if (sh.sing[buf]) { singular = true; ++gp; break; } // uniform across the cluster
-            if (owner) { // the panel's own columns now hold T e_r
-#pragma unroll
-                for (int c = 0; c < 8; ++c)
-#pragma unroll
-                    for (int sq = 0; sq < NQ; ++sq) {
-                        const double2 v = *reinterpret_cast<const double2 *>(&sh.Pn[c][64 * sq + 2 * lane]);
-                        a[2 * sq][c] = v.x;
-                        a[2 * sq + 1][c] = v.y;
-                    }
-            }
-            // ---- every thread: note the pivot rows; holders publish the OLD entries of their pivot rows
-#pragma unroll
-            for (int b = 0; b < FR_NB; ++b) {
-                const int r = sh.R[buf][b];
-                const int lane_r = (r & 63) >> 1, rr_r = 2 * (r >> 6) + (r & 1);
-                if (r == (int)threadIdx.x) used_r = true;
-                if (lane == lane_r) {
-                    if (!owner) {
-                        double2 *dst = reinterpret_cast<double2 *>(&sh.Rrow[buf][b][8 * w]);
-#pragma unroll
-                        for (int rr = 0; rr < TR; ++rr)
-                            if (rr == rr_r) {
-#pragma unroll
-                                for (int c = 0; c < 4; ++c) dst[c] = make_double2(a[rr][2 * c], a[rr][2 * c + 1]);
-                            }
-                    }
-                }
-                if (w == 0 && lane == b) { sh.rho[FR_NB * pnl + b] = r; sh.rhoinv[r] = FR_NB * pnl + b; }
-            }
-            __syncwarp(); // Rrow[.][.][8 w ..] is written and read by warp w alone
-
-            if (!owner) {
-                // ================= phase U: rank-8 update of this thread's TR x 8 tile =======================
-#pragma unroll
-                for (int b = 0; b < FR_NB; ++b) {
-                    double rv[8];
-                    const double2 *src = reinterpret_cast<const double2 *>(&sh.Rrow[buf][b][8 * w]);
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) { const double2 t = src[c]; rv[2 * c] = t.x; rv[2 * c + 1] = t.y; }
-#pragma unroll
-                    for (int s = 0; s < NQ; ++s) {
-                        const double2 z = *reinterpret_cast<const double2 *>(&sh.Z[buf][b][64 * s + 2 * lane]);
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) {
-                            a[2 * s][c] = fma(z.x, rv[c], a[2 * s][c]);
-                            a[2 * s + 1][c] = fma(z.y, rv[c], a[2 * s + 1][c]);
-                        }
-                    }
-                }
-            }
-        }
-
-        __syncthreads(); // rho / rhoinv (written by warp 0 after each panel's B1) visible to every warp of the CTA
-        double *out = Minv + (size_t)cell * n * n;
-        if (singular) {
-            if (q == 0 && threadIdx.x == 0) atomicMin(info, cell + 1);
-            // leave a NaN-free but meaningless block behind: zero this CTA's share
-            for (int e = threadIdx.x; e < 64 * n; e += FR_THREADS) out[(size_t)64 * q * n + e] = 0.0;
-            cluster_barrier(); // nobody may start the next cell's panels while a peer still reads this one's flags
-            continue;
-        }
-        // ---- store A^{-1} column-major: Ainv[rhoinv[i]][rho[j]] = W[i][j]
-        int ro[TR];
-#pragma unroll
-        for (int rr = 0; rr < TR; ++rr) ro[rr] = sh.rhoinv[64 * (rr >> 1) + 2 * lane + (rr & 1)];
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            double *col = out + (size_t)sh.rho[64 * q + 8 * w + c] * n;
-#pragma unroll
-            for (int rr = 0; rr < TR; ++rr) col[ro[rr]] = a[rr][c];
-        }
-    }
 }
 
 // ============================================================================================================
@@ -1792,60 +1499,6 @@ size_t factor_scratch_bytes(int n, int num_sms, int max_smem_optin)
     return one * (size_t)num_sms * 4;
 }
 
-template <int NQ, bool DUMP> static int launch_factor_reg_t(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
-{
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof(cfg));
-    cfg.blockDim = dim3(FR_THREADS, 1, 1);
-    cfg.dynamicSmemBytes = sizeof(FrShared<NQ>);
-    OCI_CUDA_TRY(ctx, cudaFuncSetAttribute(factor_reg_kernel<NQ, DUMP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)sizeof(FrShared<NQ>)));
-    cfg.stream = ctx->stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = NQ;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = NQ > 1 ? 1 : 0;
-    int n_clusters = 1;
-    if (!DUMP) {
-        if (NQ > 1) {
-            cfg.gridDim = dim3(NQ * ctx->num_sms, 1, 1); // any multiple of NQ: the query only needs the shape
-            OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n_clusters, factor_reg_kernel<NQ, DUMP>, &cfg));
-        } else {
-            int per_sm = 0;
-            OCI_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, factor_reg_kernel<NQ, DUMP>, FR_THREADS,
-                                                                            sizeof(FrShared<NQ>)));
-            n_clusters = per_sm * ctx->num_sms;
-        }
-        if (n_clusters < 1) n_clusters = 1;
-        if (n_clusters > ctx->J) n_clusters = ctx->J;
-    }
-    cfg.gridDim = dim3(NQ * n_clusters, 1, 1);
-    OCI_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, factor_reg_kernel<NQ, DUMP>, P, ctx->Minv, ctx->info, dumpA, dump_cell));
-    return 1;
-}
-
-// dumpA != nullptr: only assemble `dump_cell` and write the tile there
-static int launch_factor_reg_n(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
-{
-    if (dumpA) {
-        switch (ctx->n / 64) {
-        case 1: return launch_factor_reg_t<1, true>(ctx, P, dumpA, dump_cell);
-        case 2: return launch_factor_reg_t<2, true>(ctx, P, dumpA, dump_cell);
-        case 3: return launch_factor_reg_t<3, true>(ctx, P, dumpA, dump_cell);
-        default: return launch_factor_reg_t<4, true>(ctx, P, dumpA, dump_cell);
-        }
-    }
-    switch (ctx->n / 64) {
-    case 1: return launch_factor_reg_t<1, false>(ctx, P, nullptr, 0);
-    case 2: return launch_factor_reg_t<2, false>(ctx, P, nullptr, 0);
-    case 3: return launch_factor_reg_t<3, false>(ctx, P, nullptr, 0);
-    default: return launch_factor_reg_t<4, false>(ctx, P, nullptr, 0);
-    }
-}
-
 // n = 64, one warp per cell (factor_wc_kernel). dumpA != nullptr: only assemble `dump_cell` and write the tile there.
 static int launch_factor_wc(oci_ctx *ctx, const ProblemView &P, double *dumpA, int dump_cell)
 {
@@ -1968,8 +1621,6 @@ int launch_factor(oci_ctx *ctx)
     if ((ctx->opt_factor_kernel == 1 || ctx->opt_factor_kernel == 4) && n == 64) return launch_factor_wc(ctx, P, nullptr, 0);
     if (ctx->opt_factor_kernel == 1 && n == 128) return launch_factor_p128(ctx, P, nullptr, 0);
     if (ctx->opt_factor_kernel == 1 && (n == 192 || n == 256)) return launch_factor_cq(ctx, P, nullptr, 0);
-    if (ctx->opt_factor_kernel >= 1 && n % 64 == 0 && n <= 256) // 2: the 8-warp kernel also for n = 64
-        return launch_factor_reg_n(ctx, P, nullptr, 0);
     const bool global_w = factor_smem_bytes(n, false) > (size_t)ctx->max_smem_optin;
     const size_t smem = factor_smem_bytes(n, global_w);
     int grid;
@@ -2008,7 +1659,6 @@ int launch_factor_input(oci_ctx *ctx, int cell, double *A_dev_rowmajor)
         return launch_factor_wc(ctx, P, A_dev_rowmajor, cell);
     if (ctx->opt_factor_kernel == 1 && ctx->n == 128) return launch_factor_p128(ctx, P, A_dev_rowmajor, cell);
     if (ctx->opt_factor_kernel == 1 && (ctx->n == 192 || ctx->n == 256)) return launch_factor_cq(ctx, P, A_dev_rowmajor, cell);
-    if (ctx->opt_factor_kernel >= 1 && ctx->n % 64 == 0 && ctx->n <= 256) return launch_factor_reg_n(ctx, P, A_dev_rowmajor, cell);
     return 0;
 }
 

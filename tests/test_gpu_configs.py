@@ -312,7 +312,6 @@ def test_production_assembly_bit_exact(name, make):
     (16, 1, {"factor_update": 1}),     # n = 64, production kernel with one rank-8 pass per panel (default: panels paired)
     (16, 1, {"factor_kernel": 4}),     # n = 64, one warp per cell (DMMA update)
     (16, 1, {"factor_kernel": 4, "factor_update": 0}),   # n = 64, one warp per cell (DFMA update)
-    (16, 1, {"factor_kernel": 2}),     # n = 64, register-tiled cluster-capable kernel
     (8, 4, {"factor_kernel": 0}),      # n = 128, generic kernel
     (6, 8, {"factor_cluster": 1}),     # n = 192, clusters of three CTAs with eight column blocks each (default: two x 12)
     (8, 8, {"factor_cluster": 1}),     # n = 256, clusters of four CTAs (default: three, 10 + 11 + 11 blocks)

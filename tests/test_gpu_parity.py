@@ -125,18 +125,19 @@ def test_step_that_meets_a_singular_cell_leaves_a_defined_state():
 def test_option_values_outside_their_range_are_refused():
     from paper_2503_00264_b200 import OCIError
     s = _solver(W.random_problem(22, 9, 4, 1))
-    bad = {"factor_kernel": [3, 5, -1], "factor_update": [3, -1], "factor_cluster": [2], "st_consumer_threads": [64, 512],
-           "st_warp_local": [2], "st_fused_setup": [-1], "refactor_every_step": [2], "persistent": [2, -2],
-           "iterate_kernel": [2], "si_lanes": [3, 32], "solve_mode": [2], "ordering": [2], "si_sweep": [2],
-           "iterate_stages": [-1], "iterate_ctas_per_sm": [9]}
+    bad = {"factor_kernel": [2, 3, 5, -1], "factor_update": [3, -1], "factor_cluster": [2],
+           "refactor_every_step": [2], "persistent": [2, -2], "iterate_kernel": [2], "si_lanes": [3, 32],
+           "solve_mode": [2], "ordering": [2], "si_sweep": [2], "iterate_stages": [-1]}
     for key, values in bad.items():
         for v in values:
             with pytest.raises(OCIError) as e:
                 s.set_option(key, v)
             assert e.value.code == -3, (key, v)
-    with pytest.raises(OCIError) as e:
-        s.set_option("no_such_key", 0)
-    assert e.value.code == -2
+    # unknown keys, among them the tuning probes that left the public header after round 2
+    for key in ("no_such_key", "st_warp_local", "st_consumer_threads", "st_fused_setup", "iterate_ctas_per_sm"):
+        with pytest.raises(OCIError) as e:
+            s.set_option(key, 0)
+        assert e.value.code == -2, key
     for key, v in [("factor_kernel", 4), ("factor_update", 0), ("si_lanes", 16), ("persistent", -1), ("iterate_stages", 0)]:
         s.set_option(key, v)  # the documented values still pass
 
@@ -358,9 +359,9 @@ def test_si_lane_groupings_agree(lanes):
 
 
 def test_factor_kernels_agree_n64():
-    """n = 64: the two-warp kernel (default) and the eight-warp cluster-capable kernel give the same inverse to rounding."""
+    """n = 64: the two-warp kernel (default) and the generic shared-memory kernel give the same inverse to rounding."""
     p = W.config5(J=300, dt=1e-3)
-    a, b = _solver(p), _solver(p, options={"factor_kernel": 2})
+    a, b = _solver(p), _solver(p, options={"factor_kernel": 0})
     assert a.factor() == 0 and b.factor() == 0
     for j in (0, 149, 299):
         A = _oracle(p).assemble_cell(j)
