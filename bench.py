@@ -47,9 +47,9 @@ MAX_ITERS = 4000
 METRIC = "oci_cell_solves_per_s"
 UNIT = "cell-solves/s"
 # `traffic` (dram__bytes_read.sum + dram__bytes_write.sum per launch, from `ncu --set full`) is read from
-# profiles/r02_kernel_traffic.csv, which records for every capture the hash of the kernel's source files; a value is
+# profiles/r03_kernel_traffic.csv, which records for every capture the hash of the kernel's source files; a value is
 # printed only if that hash equals the hash of the sources this run was built from (ncu_traffic() below).
-TRAFFIC_FILE = "profiles/r02_kernel_traffic.csv"
+TRAFFIC_FILE = "profiles/r03_kernel_traffic.csv"
 KERNEL_SOURCES = {   # kernel -> the files (under paper_2503_00264_b200/csrc/) its code lives in
     "oci_iterate_wpc_kernel": ["iterate.cu", "common.cuh"],
     "factor_wc2_kernel": ["factor.cu", "common.cuh"],
